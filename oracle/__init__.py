@@ -1,0 +1,81 @@
+"""oracle/ -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Plain fp64 CPU oracle for the intensity-driven gradient filter (PAPER.md:165-189,
+section 3.3, Eq. 6-7), written from the paper and independent of the CUDA path:
+it imports nothing from ``paper_1609_03782_b200`` and the package imports nothing
+from here.  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s
+``cpu_baseline`` / ``--impl reference`` legs may use it.
+
+The arithmetic lives in ``idg_oracle.c`` (plain C, compiled by ``build()`` with
+gcc); this module is the ctypes loader and argument marshalling only.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = [os.path.join(_HERE, "idg_oracle.c"), os.path.join(_HERE, "ref_filters_oracle.c")]
+_LIB = os.path.join(_HERE, "libidg_oracle.so")
+_lib: Optional[ctypes.CDLL] = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle's C sources into ``oracle/libidg_oracle.so`` (gcc, -O2, OpenMP)."""
+    srcs = [s for s in _SRC if os.path.exists(s)]
+    newest = max(os.path.getmtime(s) for s in srcs)
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
+        cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp",
+               "-ffp-contract=off", "-o", _LIB] + srcs + ["-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB)
+        dp = ctypes.POINTER(ctypes.c_double)
+        lib.idg_oracle_f64.restype = ctypes.c_int
+        lib.idg_oracle_f64.argtypes = [dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                       ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                       ctypes.c_double, ctypes.c_double, ctypes.c_double, dp, dp]
+        lib.idg_oracle_set_threads.restype = ctypes.c_int
+        lib.idg_oracle_set_threads.argtypes = [ctypes.c_int]
+        _lib = lib
+    return _lib
+
+
+def set_threads(n: int) -> int:
+    """Set the OpenMP thread count of the oracle (timing only); returns the count in effect."""
+    return int(_load().idg_oracle_set_threads(int(n)))
+
+
+def idg_filter_oracle(cube: np.ndarray, n_iter: int, K: float = 1.5, tau: float = 0.0325,
+                      cx: float = 5.0, cy: float = 5.0, cz: float = 5.0,
+                      rms: float = 1.0) -> np.ndarray:
+    """n_iter IDG updates (Eq. 7) of ``cube[z, y, x]`` in fp64.
+
+    ``cube`` is indexed [z][y][x] (x = RA fastest); its values are
+    converted exactly to fp64.  Parameters are used as the fp64 values given: callers
+    comparing against the fp32 GPU path pass the fp32-rounded values (``np.float32(p)``)
+    so both sides evaluate the same function.  Returns a new fp64 array.
+    """
+    a = np.ascontiguousarray(cube, dtype=np.float64)
+    if a.ndim != 3:
+        raise ValueError("cube must be 3-D [nz, ny, nx]")
+    nz, ny, nx = a.shape
+    out = np.empty_like(a)
+    scratch = np.empty_like(a)
+    dp = ctypes.POINTER(ctypes.c_double)
+    rc = _load().idg_oracle_f64(a.ctypes.data_as(dp), nx, ny, nz, int(n_iter),
+                                float(K), float(tau), float(cx), float(cy), float(cz),
+                                float(rms), out.ctypes.data_as(dp), scratch.ctypes.data_as(dp))
+    if rc != 0:
+        raise ValueError(f"idg_oracle_f64 rejected its arguments (rc={rc})")
+    return out
