@@ -1,0 +1,152 @@
+/*
+ * idg.h -- C ABI of the B200-native intensity-driven gradient (IDG) filter.
+ *
+ * The operation is the adaptive filter of Punzo, van der Hulst & Roerdink,
+ * arXiv:1609.03782, section 3.3: n explicit steps of
+ *
+ *   I_{i+1} = I_i + tau (Cx Dx I_i + Cy Dy I_i + Cz Dz I_i) / (1 + I_i^2/(K^2 rms^2))   (Eq. 7)
+ *   Dx I    = [I(x+1,y,z) - I(x,y,z)] + [I(x-1,y,z) - I(x,y,z)]
+ *
+ * over a dense fp32 cube (RA x Dec x velocity).  The conductance (Eq. 6,
+ * PAPER.md:178) is evaluated at the centre voxel of the current iterate; the
+ * update is Jacobi (two buffers); an out-of-cube neighbour
+ * equals the centre voxel (zero-flux boundary, reading R1); rms is a
+ * caller-supplied constant.  All arithmetic runs in hand-written sm_100a CUDA
+ * kernels; there is no CPU fallback.
+ *
+ * Conventions for every entry point
+ *   layout    dense, idx = x + nx*(y + ny*z); x = RA (fastest), y = Dec,
+ *             z = velocity (slowest); batched cubes are contiguous, stride nx*ny*nz.
+ *   pointers  marked [device] or [host].  All buffers are caller-owned; the
+ *             library never frees or keeps them.  `cube` is read-only unless
+ *             out == cube (in place is allowed); otherwise cube/out/workspace
+ *             must not overlap.
+ *   stream    a cudaStream_t passed as void* (NULL = legacy default stream).
+ *             All device work is enqueued on it; calls do not synchronise the
+ *             host except where stated (idg_filter_host).
+ *   return    0 = IDG_OK; negative = argument error found on the host before
+ *             any launch (nothing was enqueued); positive = a cudaError_t.
+ *   NaN       voxels propagate by IEEE rules (FITS blanks are not treated).
+ */
+#ifndef IDG_H_
+#define IDG_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define IDG_VERSION 100            /* major*10000 + minor*100 + patch */
+
+enum {
+    IDG_OK = 0,
+    IDG_ERR_NULL = -1,             /* a required pointer is NULL */
+    IDG_ERR_DIMS = -2,             /* nx, ny, nz or batch < 1, or voxel count overflows */
+    IDG_ERR_NITER = -3,            /* n_iter < 0 */
+    IDG_ERR_PARAM = -4,            /* K <= 0 or NaN; tau, Cj < 0; rms <= 0; non-finite (K = +inf is allowed) */
+    IDG_ERR_WORKSPACE = -5,        /* workspace NULL, too small or not 256-byte aligned */
+    IDG_ERR_OVERLAP = -6,          /* cube/out/workspace partially overlap */
+    IDG_ERR_OPTION = -7            /* unknown option key or value out of range */
+};
+
+/*
+ * Filter parameters.  Paper GUI ranges: tau in [0.0025, 0.0625],
+ * Cj in [0, 10], K in [0.5, 10]; defaults K = 1.5, tau = 0.0325, Cj = 5, n = 20.
+ * Values outside the ranges are accepted (idg_params_check reports them).
+ */
+typedef struct idg_params {
+    float K;            /* conductance scale in units of rms; > 0; +INFINITY = constant conductance */
+    float tau;          /* time step; >= 0 */
+    float cx, cy, cz;   /* axis weights Cx (RA), Cy (Dec), Cz (velocity); >= 0 */
+    float rms;          /* noise level of the ORIGINAL cube, in cube units; > 0; constant over iterations */
+} idg_params;
+
+/* Library version (IDG_VERSION of the build). */
+int idg_version(void);
+
+/* Static, NUL-terminated description of a status returned by any entry point. */
+const char *idg_status_string(int status);
+
+/*
+ * Host-only check of one parameter set.  Returns a bit mask:
+ *   bit 0  some value lies outside the paper's GUI range
+ *   bit 1  tau*(Cx+Cy+Cz) > 1/2: the explicit scheme is linearly unstable where
+ *          the conductance is ~1 (reading R9)
+ *   bit 2  the set is invalid (the filter entry points would return IDG_ERR_PARAM)
+ */
+unsigned idg_params_check(const idg_params *params /*[host]*/);
+
+/*
+ * Bytes of device workspace idg_filter_ws / idg_filter_batched need for `batch`
+ * cubes of nx*ny*nz voxels: one scratch cube per cube (the "temporary eta" of
+ * PAPER.md:430) plus a small parameter table.  0 on invalid dimensions.
+ */
+size_t idg_workspace_bytes(int nx, int ny, int nz, int batch);
+
+/*
+ * n_iter IDG updates (Eq. 7) of one cube.  north_star signature: the scratch
+ * cube is taken from the stream-ordered allocator (cudaMallocAsync on `stream`)
+ * and returned to it before the call returns.
+ *   cube   [device] nx*ny*nz fp32, input I_0
+ *   params [host]   one idg_params, copied during the call
+ *   out    [device] nx*ny*nz fp32, receives I_n (n_iter = 0 copies cube)
+ */
+int idg_filter(const float *cube, int nx, int ny, int nz, int n_iter,
+               const idg_params *params, float *out, void *stream);
+
+/*
+ * As idg_filter, never allocating: `workspace` [device] must hold
+ * idg_workspace_bytes(nx, ny, nz, 1) bytes, 256-byte aligned.
+ */
+int idg_filter_ws(const float *cube, int nx, int ny, int nz, int n_iter,
+                  const idg_params *params, float *out,
+                  void *workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * `batch` independent cubes of equal shape in one call (interactive parameter
+ * exploration), each with its own parameters and
+ * iteration count.
+ *   cubes  [device] batch*nx*ny*nz fp32
+ *   n_iter [host]   batch ints (each >= 0), or NULL to use n_iter_all for all
+ *   params [host]   batch idg_params
+ *   out    [device] batch*nx*ny*nz fp32 (may equal cubes)
+ *   workspace [device] idg_workspace_bytes(nx, ny, nz, batch) bytes, 256-byte aligned
+ */
+int idg_filter_batched(const float *cubes, int nx, int ny, int nz, int batch,
+                       const int *n_iter, int n_iter_all, const idg_params *params,
+                       float *out, void *workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * End-to-end convenience for HOST buffers (the paper's T_p includes the
+ * transfers): copies cube_host to the device, filters, copies
+ * I_n to out_host and synchronises `stream` before returning.
+ *   cube_host, out_host [host] nx*ny*nz fp32 (pinned memory gives full PCIe rate)
+ *   dev_buffers [device] 2*nx*ny*nz*4 + idg_workspace_bytes(nx,ny,nz,1) bytes,
+ *               256-byte aligned, or NULL to use the stream-ordered allocator.
+ */
+int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
+                    const idg_params *params, float *out_host,
+                    void *dev_buffers, size_t dev_buffers_bytes, void *stream);
+
+/*
+ * Process-wide tuning knobs (tests and benchmarks; defaults give the fastest plan).
+ *   IDG_OPT_KERNEL   0 auto | 1 naive (one thread per voxel) | 2 tiled z-streaming kernel
+ *   IDG_OPT_FUSE     0 auto | 1..4 = diffusion iterations fused per launch (tiled kernel)
+ *   IDG_OPT_ZCHUNK   0 auto | >0  = planes per CTA along z (tiled kernel)
+ * idg_get_option returns the current value, or IDG_ERR_OPTION.
+ */
+enum { IDG_OPT_KERNEL = 0, IDG_OPT_FUSE = 1, IDG_OPT_ZCHUNK = 2, IDG_OPT_COUNT_ = 3 };
+int idg_set_option(int key, int value);
+int idg_get_option(int key);
+
+/*
+ * Number of kernel launches the last filter call on this thread enqueued
+ * (for bench.py's "gpu_launches" claim).
+ */
+int idg_last_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IDG_H_ */

@@ -1,0 +1,216 @@
+"""ctypes binding of libidg_b200.so (include/idg.h): argument marshalling only.
+
+Same names as the C ABI.  torch supplies device memory and streams; every voxel
+update runs in the library's CUDA kernels.  There is no CPU path: a missing
+library or a CPU tensor raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional, Sequence, Union
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libidg_b200.so")
+
+IDG_OPT_KERNEL, IDG_OPT_FUSE, IDG_OPT_ZCHUNK = 0, 1, 2
+KERNEL_AUTO, KERNEL_NAIVE, KERNEL_TILED = 0, 1, 2
+
+# every symbol include/idg.h declares (tests check the library exports them all)
+SYMBOLS = ("idg_version", "idg_status_string", "idg_params_check", "idg_workspace_bytes",
+           "idg_filter", "idg_filter_ws", "idg_filter_batched", "idg_filter_host",
+           "idg_set_option", "idg_get_option", "idg_last_launch_count")
+
+
+class IdgParams(ctypes.Structure):
+    """struct idg_params: K, tau, cx, cy, cz, rms -- all fp32."""
+    _fields_ = [("K", ctypes.c_float), ("tau", ctypes.c_float), ("cx", ctypes.c_float),
+                ("cy", ctypes.c_float), ("cz", ctypes.c_float), ("rms", ctypes.c_float)]
+
+
+@dataclass
+class Params:
+    """Paper defaults: K = 1.5, tau = 0.0325, Cx = Cy = Cz = 5."""
+    K: float = 1.5
+    tau: float = 0.0325
+    cx: float = 5.0
+    cy: float = 5.0
+    cz: float = 5.0
+    rms: float = 1.0
+
+    def c(self) -> IdgParams:
+        return IdgParams(self.K, self.tau, self.cx, self.cy, self.cz, self.rms)
+
+    def f32(self) -> dict:
+        """The fp32-rounded values the library sees, as Python floats (for the oracle)."""
+        return {k: float(np.float32(getattr(self, k))) for k in ("K", "tau", "cx", "cy", "cz", "rms")}
+
+
+class IdgError(RuntimeError):
+    def __init__(self, status: int):
+        self.status = status
+        super().__init__(f"idg status {status}: {status_string(status)}")
+
+
+_lib: Optional[ctypes.CDLL] = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libidg_b200.so; fails loudly if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_1609_03782_b200.build` "
+                               "(the IDG filter has no CPU or PyTorch fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, fp, ip, sz, i = ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int
+        pp = ctypes.POINTER(IdgParams)
+        L.idg_version.restype = i
+        L.idg_status_string.restype = ctypes.c_char_p
+        L.idg_status_string.argtypes = [i]
+        L.idg_params_check.restype = ctypes.c_uint
+        L.idg_params_check.argtypes = [pp]
+        L.idg_workspace_bytes.restype = sz
+        L.idg_workspace_bytes.argtypes = [i, i, i, i]
+        L.idg_filter.restype = i
+        L.idg_filter.argtypes = [fp, i, i, i, i, pp, fp, vp]
+        L.idg_filter_ws.restype = i
+        L.idg_filter_ws.argtypes = [fp, i, i, i, i, pp, fp, vp, sz, vp]
+        L.idg_filter_batched.restype = i
+        L.idg_filter_batched.argtypes = [fp, i, i, i, i, ip, i, pp, fp, vp, sz, vp]
+        L.idg_filter_host.restype = i
+        L.idg_filter_host.argtypes = [fp, i, i, i, i, pp, fp, vp, sz, vp]
+        L.idg_set_option.restype = i
+        L.idg_set_option.argtypes = [i, i]
+        L.idg_get_option.restype = i
+        L.idg_get_option.argtypes = [i]
+        L.idg_last_launch_count.restype = i
+        _lib = L
+    return _lib
+
+
+def _check(status: int) -> None:
+    if status != 0:
+        raise IdgError(status)
+
+
+def _dev(t: torch.Tensor, name: str) -> int:
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name} must be a CUDA tensor (no CPU path)")
+    if t.dtype != torch.float32 or not t.is_contiguous():
+        raise TypeError(f"{name} must be a contiguous float32 tensor")
+    return t.data_ptr()
+
+
+def _stream(stream: Optional[torch.cuda.Stream]) -> int:
+    return (stream or torch.cuda.current_stream()).cuda_stream
+
+
+def idg_version() -> int:
+    return int(lib().idg_version())
+
+
+def status_string(status: int) -> str:
+    return lib().idg_status_string(int(status)).decode()
+
+
+def idg_params_check(p: Params) -> int:
+    c = p.c()
+    return int(lib().idg_params_check(ctypes.byref(c)))
+
+
+def idg_workspace_bytes(nx: int, ny: int, nz: int, batch: int = 1) -> int:
+    return int(lib().idg_workspace_bytes(nx, ny, nz, batch))
+
+
+def idg_set_option(key: int, value: int) -> None:
+    _check(lib().idg_set_option(key, value))
+
+
+def idg_get_option(key: int) -> int:
+    return int(lib().idg_get_option(key))
+
+
+def idg_last_launch_count() -> int:
+    return int(lib().idg_last_launch_count())
+
+
+def alloc_workspace(nx: int, ny: int, nz: int, batch: int = 1, device="cuda") -> torch.Tensor:
+    return torch.empty(idg_workspace_bytes(nx, ny, nz, batch), dtype=torch.uint8, device=device)
+
+
+def idg_filter(cube: torch.Tensor, n_iter: int, params: Params = Params(),
+               out: Optional[torch.Tensor] = None, workspace: Optional[torch.Tensor] = None,
+               stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """idg_filter / idg_filter_ws on a [nz, ny, nx] CUDA tensor.  Asynchronous on `stream`."""
+    if cube.dim() != 3:
+        raise ValueError("cube must be [nz, ny, nx]")
+    nz, ny, nx = cube.shape
+    if out is None:
+        out = torch.empty_like(cube)
+    c = params.c()
+    if workspace is None:
+        rc = lib().idg_filter(_dev(cube, "cube"), nx, ny, nz, int(n_iter), ctypes.byref(c),
+                              _dev(out, "out"), _stream(stream))
+    else:
+        rc = lib().idg_filter_ws(_dev(cube, "cube"), nx, ny, nz, int(n_iter), ctypes.byref(c),
+                                 _dev(out, "out"), workspace.data_ptr(), workspace.numel(),
+                                 _stream(stream))
+    _check(rc)
+    return out
+
+
+def idg_filter_batched(cubes: torch.Tensor, n_iter: Union[int, Sequence[int]],
+                       params: Sequence[Params], out: Optional[torch.Tensor] = None,
+                       workspace: Optional[torch.Tensor] = None,
+                       stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """idg_filter_batched on a [B, nz, ny, nx] CUDA tensor with per-cube parameters."""
+    if cubes.dim() != 4:
+        raise ValueError("cubes must be [B, nz, ny, nx]")
+    B, nz, ny, nx = cubes.shape
+    if len(params) != B:
+        raise ValueError("one Params per cube")
+    if out is None:
+        out = torch.empty_like(cubes)
+    if workspace is None:
+        workspace = alloc_workspace(nx, ny, nz, B, cubes.device)
+    arr = (IdgParams * B)(*[p.c() for p in params])
+    if isinstance(n_iter, int):
+        n_ptr, n_all = None, n_iter
+    else:
+        if len(n_iter) != B:
+            raise ValueError("one n_iter per cube")
+        n_arr = (ctypes.c_int * B)(*[int(v) for v in n_iter])
+        n_ptr, n_all = ctypes.cast(n_arr, ctypes.c_void_p), 0
+    rc = lib().idg_filter_batched(_dev(cubes, "cubes"), nx, ny, nz, B, n_ptr, n_all, arr,
+                                  _dev(out, "out"), workspace.data_ptr(), workspace.numel(),
+                                  _stream(stream))
+    _check(rc)
+    return out
+
+
+def idg_filter_host(cube_host: torch.Tensor, n_iter: int, params: Params = Params(),
+                    out_host: Optional[torch.Tensor] = None,
+                    dev_buffers: Optional[torch.Tensor] = None,
+                    stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """idg_filter_host: HOST fp32 tensors in and out (pinned for full PCIe rate); synchronises."""
+    if cube_host.is_cuda or cube_host.dtype != torch.float32 or not cube_host.is_contiguous():
+        raise TypeError("cube_host must be a contiguous float32 CPU tensor")
+    nz, ny, nx = cube_host.shape
+    if out_host is None:
+        out_host = torch.empty_like(cube_host, pin_memory=cube_host.is_pinned())
+    c = params.c()
+    dptr, dbytes = (dev_buffers.data_ptr(), dev_buffers.numel()) if dev_buffers is not None else (None, 0)
+    rc = lib().idg_filter_host(cube_host.data_ptr(), nx, ny, nz, int(n_iter), ctypes.byref(c),
+                               out_host.data_ptr(), dptr, dbytes, _stream(stream))
+    _check(rc)
+    return out_host
+
+
+def host_buffers_bytes(nx: int, ny: int, nz: int) -> int:
+    cube = (nx * ny * nz * 4 + 255) // 256 * 256
+    return 2 * cube + idg_workspace_bytes(nx, ny, nz, 1)

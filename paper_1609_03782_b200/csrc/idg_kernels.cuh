@@ -1,0 +1,85 @@
+// Internal declarations shared by the CUDA translation units of libidg_b200.so.
+// Not part of the public boundary (include/idg.h) and not used by oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace idg {
+
+// Per-cube constants derived on the host in fp64 and rounded once (step a0):
+//   ax = tau*Cx, ay = tau*Cy, az = tau*Cz   (Eq. 7 numerator)
+//   s  = 1/(K*rms), 0 when K = +inf         (Eq. 6:  S = 1/(1 + (I*s)^2))
+struct CubeParams {
+    float ax, ay, az, s;
+    int n_iter;
+    int pad_[3];
+};
+static_assert(sizeof(CubeParams) == 32, "CubeParams is uploaded as a 32-byte record");
+
+// One launch over `batch` cubes; iterations [iter_done, iter_done + fuse) of each cube that
+// still has iterations left.
+struct Launch {
+    const float *in;        // I_0 of cube 0 (read only by each cube's first launch)
+    float *out;             // final destination of cube 0
+    float *scratch;         // scratch cube 0
+    const CubeParams *tab;  // device table [batch], or nullptr -> use `one`
+    CubeParams one;
+    int nx, ny, nz, batch;
+    int iter_done;          // iterations already applied to every cube by earlier launches
+    int fuse;               // iterations per launch of this plan (T)
+    int in_place;           // out == in: the host staged a copy of I_0 in `scratch`
+};
+
+// Which buffers cube b reads / writes in this launch so that its LAST launch writes `out`.
+// Returns the number of iterations to apply now (0 = cube already finished).
+__device__ __forceinline__ int route(const Launch &L, int b, const CubeParams &p,
+                                     const float *&src, float *&dst)
+{
+    const int remaining = p.n_iter - L.iter_done;
+    if (remaining <= 0) return 0;
+    const int now = remaining < L.fuse ? remaining : L.fuse;
+    const int after = (remaining - now + L.fuse - 1) / L.fuse;      // launches still to come
+    const size_t off = (size_t)b * (size_t)L.nx * (size_t)L.ny * (size_t)L.nz;
+    float *o = L.out + off, *s = L.scratch + off;
+    dst = (after & 1) ? s : o;
+    if (L.iter_done == 0)   // first launch: read I_0 (from the staged copy if it would alias dst)
+        src = (L.in_place && !(after & 1)) ? s : (L.in + off);
+    else
+        src = (after & 1) ? o : s;
+    return now;
+}
+
+__device__ __forceinline__ CubeParams cube_params(const Launch &L, int b)
+{
+    return L.tab ? L.tab[b] : L.one;
+}
+
+// Conductance S = 1/(1 + u^2), u = I*s  (Eq. 6).  den >= 1, so the approximate reciprocal
+// (one MUFU.RCP, <= 1 ulp) needs no range handling; rcp(1) == 1 exactly (K = +inf limit).
+__device__ __forceinline__ float conductance(float c, float s)
+{
+    const float u = c * s;
+    const float den = fmaf(u, u, 1.0f);
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(den));
+    return r;
+}
+
+// One voxel update (Eq. 7).  Differences are formed as (xp + xm) - 2c: exact zero for a
+// constant neighbourhood, so a constant cube is a bitwise fixed point.
+__device__ __forceinline__ float update(float c, float xm, float xp, float ym, float yp,
+                                        float zm, float zp, float ax, float ay, float az, float s)
+{
+    const float dx = fmaf(-2.0f, c, xp + xm);
+    const float dy = fmaf(-2.0f, c, yp + ym);
+    const float dz = fmaf(-2.0f, c, zp + zm);
+    const float lap = fmaf(az, dz, fmaf(ay, dy, ax * dx));
+    return fmaf(lap, conductance(c, s), c);
+}
+
+// Kernel launchers (each returns cudaGetLastError of its launch).
+cudaError_t launch_naive(const Launch &L, cudaStream_t st);
+cudaError_t launch_tiled(const Launch &L, int zchunk, cudaStream_t st);
+bool tiled_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
+
+}  // namespace idg

@@ -1,0 +1,316 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element.
+
+Bar (BASELINE.json north_star): max |gpu - oracle| <= 1e-4 * noise rms after the configured
+iteration count.  Inputs come from paper_1609_03782_b200.synth (seeded) or a seeded normal
+draw; the oracle receives the same fp32 values and the fp32-rounded parameters.
+"""
+import math
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4          # x rms  (north_star)
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1609_03782_b200 import binding
+    binding.lib()           # fails loudly if the extension is missing
+    yield binding
+    for k in (binding.IDG_OPT_KERNEL, binding.IDG_OPT_FUSE, binding.IDG_OPT_ZCHUNK):
+        binding.idg_set_option(k, 0)
+
+
+# (kernel, fuse) plans every parity case runs under
+PLANS = [(1, 0), (2, 1), (2, 2), (2, 3), (2, 4), (0, 0)]
+PLAN_IDS = ["naive", "tiled-T1", "tiled-T2", "tiled-T3", "tiled-T4", "auto"]
+
+
+def set_plan(B, plan, zchunk=0):
+    B.idg_set_option(B.IDG_OPT_KERNEL, plan[0])
+    B.idg_set_option(B.IDG_OPT_FUSE, plan[1])
+    B.idg_set_option(B.IDG_OPT_ZCHUNK, zchunk)
+
+
+def gpu(B, cube_np, n, p, **kw):
+    t = torch.from_numpy(np.ascontiguousarray(cube_np, dtype=np.float32)).cuda()
+    out = B.idg_filter(t, n, p, **kw)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def err(out, ref, rms):
+    return float(np.abs(out.astype(np.float64) - ref).max()) / rms
+
+
+SHAPES = [(1, 1, 1), (1, 1, 13), (13, 1, 1), (1, 9, 1), (4, 4, 4), (7, 6, 5), (3, 5, 8), (2, 3, 260),
+          (9, 70, 132), (5, 33, 45), (21, 67, 100), (6, 130, 12)]
+
+
+@pytest.mark.parametrize("plan", PLANS, ids=PLAN_IDS)
+@pytest.mark.parametrize("shape", SHAPES, ids=lambda s: "x".join(map(str, s[::-1])))
+def test_small_shapes(B, oracle, plan, shape):
+    """Tiny, odd and degenerate shapes (nx not a multiple of 4, nz < T, size-1 axes)."""
+    set_plan(B, plan)
+    rng = np.random.default_rng(hash(shape) % 2 ** 31)
+    a = (rng.normal(0, 1, shape) + 8.0 * (rng.random(shape) < 0.05)).astype(np.float32)
+    p = B.Params(K=1.5, tau=0.0325, cx=5.0, cy=4.0, cz=6.0, rms=1.0)
+    for n in (0, 1, 2, 5, 10):
+        ref = oracle.idg_filter_oracle(a, n, **p.f32())
+        out = gpu(B, a, n, p)
+        assert err(out, ref, 1.0) <= TOL, (shape, n)
+
+
+@pytest.mark.parametrize("plan", PLANS, ids=PLAN_IDS)
+def test_config0_full_cube(B, oracle, plan):
+    """configs[0]: 100x100x67, S/N 32, defaults, n = 10; full cube."""
+    from paper_1609_03782_b200 import synth
+    set_plan(B, plan)
+    c = synth.modelb_like(seed=1000, snr=32.0)
+    p = B.Params()
+    ref = oracle.idg_filter_oracle(c.data, 10, **p.f32())
+    out = gpu(B, c.data, 10, p)
+    assert err(out, ref, c.rms) <= TOL
+
+
+@pytest.mark.parametrize("zchunk", [1, 3, 16, 1000])
+@pytest.mark.parametrize("fuse", [1, 2, 4])
+def test_zchunk_variants(B, oracle, fuse, zchunk):
+    """z-chunking of the tiled kernel (ragged last chunk, chunk < T, chunk > nz)."""
+    set_plan(B, (2, fuse), zchunk)
+    rng = np.random.default_rng(5)
+    a = rng.normal(0, 2, (19, 70, 136)).astype(np.float32)
+    p = B.Params(K=2.0, tau=0.03, cx=5.0, cy=5.0, cz=5.0, rms=2.0)
+    ref = oracle.idg_filter_oracle(a, 7, **p.f32())
+    assert err(gpu(B, a, 7, p), ref, 2.0) <= TOL
+
+
+def test_config1_parameter_sweep(B, oracle):
+    """configs[1]: S/N 22 and 62 cubes, 8 K values, n = 1..40 (snapshots at 1, 5, 10, 20, 40 here;
+    the oracle runs incrementally -- Markov property, pinned by test_p11)."""
+    from paper_1609_03782_b200 import synth
+    set_plan(B, (0, 0))
+    for seed, snr in ((1001, 22.0), (1002, 62.0)):
+        c = synth.modelb_like(seed=seed, snr=snr)
+        assert c.peak < 64.0, "fp32 rounding floor argument needs max|I| < 64 rms (DESIGN.md section 6)"
+        for K in synth.K_SWEEP:
+            p = B.Params(K=K)
+            ref, done = c.data.astype(np.float64), 0
+            for n in (1, 5, 10, 20, 40):
+                ref = oracle.idg_filter_oracle(ref, n - done, **p.f32())
+                done = n
+                assert err(gpu(B, c.data, n, p), ref, c.rms) <= TOL, (snr, K, n)
+
+
+def test_incremental_equals_from_scratch(B):
+    """f(I, n+m) == f(f(I, n), m): the n-sweep may be run incrementally."""
+    from paper_1609_03782_b200 import synth
+    set_plan(B, (2, 1))
+    c = synth.modelb_like(seed=1001, snr=22.0)
+    p = B.Params()
+    t = torch.from_numpy(c.data).cuda()
+    a = B.idg_filter(B.idg_filter(t, 4, p), 6, p)
+    b = B.idg_filter(t, 10, p)
+    assert torch.equal(a, b)           # same kernel, one iteration per launch: bitwise
+
+
+def sub_blocks(shape, n, B_in, count, rng):
+    """Sub-blocks (z0,z1,y0,y1,x0,x1) with margin n whose inner B_in^3 is exact (domain of
+    dependence, pinned by test_p8); the first ones hug all 8 corners."""
+    nz, ny, nx = shape
+    size = B_in + 2 * n
+    starts = []
+    for cz in (0, nz - size):
+        for cy in (0, ny - size):
+            for cx in (0, nx - size):
+                starts.append((max(cz, 0), max(cy, 0), max(cx, 0)))
+    while len(starts) < count:
+        starts.append(tuple(int(rng.integers(0, max(d - size, 0) + 1)) for d in (nz, ny, nx)))
+    return [(z, min(z + size, nz), y, min(y + size, ny), x, min(x + size, nx)) for z, y, x in starts]
+
+
+def check_blocks(oracle, cube, out, n, p, blocks, rms):
+    worst = 0.0
+    for (z0, z1, y0, y1, x0, x1) in blocks:
+        ref = oracle.idg_filter_oracle(cube[z0:z1, y0:y1, x0:x1], n, **p.f32())
+        # a side of the block that is a true cube face keeps its face; others lose n voxels
+        lo = [0 if s == 0 else n for s in (z0, y0, x0)]
+        hi = [(e - s) if e == full else (e - s - n)
+              for s, e, full in ((z0, z1, cube.shape[0]), (y0, y1, cube.shape[1]), (x0, x1, cube.shape[2]))]
+        sl = tuple(slice(a, b) for a, b in zip(lo, hi))
+        g = out[z0:z1, y0:y1, x0:x1][sl]
+        worst = max(worst, err(g, ref[sl], rms))
+    return worst
+
+
+def test_config2_survey_field(B, oracle):
+    """configs[2]: 512x512x256, 6 discs, defaults, n = 20; 40 sub-blocks incl. all corners, plus
+    the block around the brightest voxel."""
+    from paper_1609_03782_b200 import synth
+    set_plan(B, (0, 0))
+    c = synth.survey_field((256, 512, 512), seed=2000, n_discs=6)
+    p = B.Params()
+    out = gpu(B, c.data, 20, p)
+    rng = np.random.default_rng(2)
+    blocks = sub_blocks(c.data.shape, 20, 24, 40, rng)
+    bz, by, bx = np.unravel_index(np.argmax(c.data), c.data.shape)
+    blocks.append((max(bz - 32, 0), min(bz + 32, 256), max(by - 32, 0), min(by + 32, 512),
+                   max(bx - 32, 0), min(bx + 32, 512)))
+    assert check_blocks(oracle, c.data, out, 20, p, blocks, c.rms) <= TOL
+
+
+def test_config3_large_cube(B, oracle):
+    """configs[3]: 1024x1024x512 (2.1 GB), 20 discs + extra-planar gas, defaults, n = 20, in the
+    launch configuration bench.py times (auto plan, workspace variant).  The oracle cannot hold
+    the full cube in seconds, so 48 sub-blocks (all 8 corners, faces, random interior, brightest
+    voxel) are compared on their exact inner region."""
+    from paper_1609_03782_b200 import synth
+    free, _ = torch.cuda.mem_get_info()
+    if free < 8 * 2 ** 30:
+        pytest.skip("needs 8 GB of device memory")
+    set_plan(B, (0, 0))
+    c = synth.large_cube(seed=3000)
+    p = B.Params()
+    t = torch.from_numpy(c.data).cuda()
+    ws = B.alloc_workspace(1024, 1024, 512, 1)
+    o = B.idg_filter(t, 20, p, workspace=ws)
+    torch.cuda.synchronize()
+    out = o.cpu().numpy()
+    rng = np.random.default_rng(3)
+    blocks = sub_blocks(c.data.shape, 20, 24, 47, rng)
+    bz, by, bx = np.unravel_index(np.argmax(c.data), c.data.shape)
+    blocks.append((max(bz - 32, 0), min(bz + 32, 512), max(by - 32, 0), min(by + 32, 1024),
+                   max(bx - 32, 0), min(bx + 32, 1024)))
+    assert check_blocks(oracle, c.data, out, 20, p, blocks, c.rms) <= TOL
+    assert np.isfinite(out).all()
+
+
+def test_config4_batched(B, oracle):
+    """configs[4]: 128x128x64 cubes with per-cube parameters, n = 10, one batched call.
+    32 cubes against the oracle; all of them against single-cube calls bitwise."""
+    from paper_1609_03782_b200 import synth
+    set_plan(B, (0, 0))
+    nb = 32
+    cubes = synth.batch_cubes(nb, seed=4000)
+    prm = synth.batch_params(256, seed=4000)[:nb]
+    ps = [B.Params(*[float(v) for v in row]) for row in prm]
+    t = torch.from_numpy(cubes).cuda()
+    out = B.idg_filter_batched(t, 10, ps)
+    torch.cuda.synchronize()
+    o = out.cpu().numpy()
+    for b in range(nb):
+        ref = oracle.idg_filter_oracle(cubes[b], 10, **ps[b].f32())
+        assert err(o[b], ref, 1.0) <= TOL, b
+        single = B.idg_filter(t[b], 10, ps[b])
+        assert torch.equal(single, out[b]), b
+
+
+def test_batched_mixed_iteration_counts(B, oracle):
+    """Per-cube n_iter (including 0 and counts that are not multiples of T), in place and not."""
+    rng = np.random.default_rng(11)
+    cubes = rng.normal(0, 1.5, (7, 9, 20, 24)).astype(np.float32)
+    ns = [0, 1, 2, 3, 7, 10, 4]
+    ps = [B.Params(K=0.5 + b, tau=0.02, cx=4 + (b % 3), cy=5.0, cz=6.0, rms=1.5) for b in range(7)]
+    for plan in PLANS:
+        set_plan(B, plan)
+        t = torch.from_numpy(cubes).cuda()
+        out = B.idg_filter_batched(t, ns, ps)
+        inpl = t.clone()
+        B.idg_filter_batched(inpl, ns, ps, out=inpl)
+        torch.cuda.synchronize()
+        for b in range(7):
+            ref = oracle.idg_filter_oracle(cubes[b], ns[b], **ps[b].f32())
+            assert err(out[b].cpu().numpy(), ref, 1.5) <= TOL, (plan, b)
+            assert torch.equal(out[b], inpl[b]), (plan, b)
+        assert torch.equal(t, torch.from_numpy(cubes).cuda())     # input untouched
+
+
+@pytest.mark.parametrize("plan", PLANS, ids=PLAN_IDS)
+def test_invariants_bitwise(B, plan):
+    """On the GPU output directly: constant cube fixed point, odd symmetry, power-of-two scale
+    covariance -- all bitwise in fp32."""
+    set_plan(B, plan)
+    p = B.Params(K=1.5, tau=0.0325, cx=5.0, cy=3.0, cz=6.0, rms=1.0)
+    const = torch.full((9, 20, 36), 7.3, device="cuda")
+    assert torch.equal(B.idg_filter(const, 6, p), const)
+    g = torch.Generator(device="cpu").manual_seed(3)
+    a = (torch.randn(9, 20, 36, generator=g) * 3).cuda()
+    f = B.idg_filter(a, 6, p)
+    assert torch.equal(B.idg_filter(-a, 6, p), -f)
+    q = B.Params(K=1.5, tau=0.0325, cx=5.0, cy=3.0, cz=6.0, rms=8.0)
+    assert torch.equal(B.idg_filter(a * 8, 6, q), f * 8)
+
+
+def test_linear_limit_conserves_sum_on_gpu(B):
+    """K = +inf: conductance exactly 1; the voxel sum is conserved to fp32 rounding."""
+    set_plan(B, (0, 0))
+    g = torch.Generator(device="cpu").manual_seed(4)
+    a = torch.randn(16, 40, 64, generator=g).cuda()
+    f = B.idg_filter(a, 20, B.Params(K=math.inf))
+    assert abs(f.double().sum().item() - a.double().sum().item()) < 1e-3
+    assert f.std().item() < 0.5 * a.std().item()
+
+
+def test_in_place_and_workspace_variants(B, oracle):
+    rng = np.random.default_rng(8)
+    a = rng.normal(0, 1, (10, 24, 40)).astype(np.float32)
+    p = B.Params()
+    for plan in PLANS:
+        set_plan(B, plan)
+        for n in (1, 2, 3, 4, 5):
+            ref = oracle.idg_filter_oracle(a, n, **p.f32())
+            t = torch.from_numpy(a).cuda()
+            B.idg_filter(t, n, p, out=t)                          # in place, allocator variant
+            assert err(t.cpu().numpy(), ref, 1.0) <= TOL
+            t = torch.from_numpy(a).cuda()
+            ws = B.alloc_workspace(40, 24, 10)
+            B.idg_filter(t, n, p, out=t, workspace=ws)            # in place, workspace variant
+            assert err(t.cpu().numpy(), ref, 1.0) <= TOL
+
+
+def test_host_entry_point(B, oracle):
+    """idg_filter_host: host buffers in and out, copies inside the call."""
+    from paper_1609_03782_b200 import synth
+    set_plan(B, (0, 0))
+    c = synth.modelb_like(seed=1000, snr=32.0)
+    p = B.Params()
+    h = torch.from_numpy(c.data).pin_memory()
+    out = B.idg_filter_host(h, 10, p)
+    ref = oracle.idg_filter_oracle(c.data, 10, **p.f32())
+    assert err(out.numpy(), ref, 1.0) <= TOL
+    dev = torch.empty(B.host_buffers_bytes(100, 100, 67), dtype=torch.uint8, device="cuda")
+    out2 = B.idg_filter_host(h, 10, p, dev_buffers=dev)
+    assert torch.equal(out, out2)
+
+
+def test_argument_errors(B):
+    from paper_1609_03782_b200.binding import IdgError
+    t = torch.zeros(4, 4, 4, device="cuda")
+    with pytest.raises(IdgError) as e:
+        B.idg_filter(t, -1)
+    assert e.value.status == -3
+    with pytest.raises(IdgError) as e:
+        B.idg_filter(t, 1, B.Params(K=0.0))
+    assert e.value.status == -4
+    with pytest.raises(IdgError) as e:
+        B.idg_filter(t, 1, workspace=torch.empty(16, dtype=torch.uint8, device="cuda"))
+    assert e.value.status == -5
+    big = torch.zeros(2 * 64 + 8, device="cuda")
+    with pytest.raises(IdgError) as e:           # partial overlap of cube and out
+        B.idg_filter(big[:64].view(4, 4, 4), 1, out=big[8:72].view(4, 4, 4))
+    assert e.value.status == -6
+
+
+def test_launch_count(B):
+    set_plan(B, (1, 0))
+    t = torch.zeros(4, 8, 8, device="cuda")
+    B.idg_filter(t, 7)
+    assert B.idg_last_launch_count() == 7
+    set_plan(B, (2, 2))
+    B.idg_filter(t, 7)
+    assert B.idg_last_launch_count() == 4
