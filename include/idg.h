@@ -131,9 +131,10 @@ int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
 
 /*
  * Process-wide tuning knobs (tests and benchmarks; defaults give the fastest plan).
- *   IDG_OPT_KERNEL   0 auto | 1 naive (one thread per voxel) | 2 tiled z-streaming kernel
- *   IDG_OPT_FUSE     0 auto | 1..4 = diffusion iterations fused per launch (tiled kernel)
- *   IDG_OPT_ZCHUNK   0 auto | >0  = planes per CTA along z (tiled kernel)
+ *   IDG_OPT_KERNEL   0 auto | 1 naive (one thread per voxel) | 2 tiled z-streaming kernel (global loads)
+ *                    | 3 tiled z-streaming kernel fed by TMA (the fast path)
+ *   IDG_OPT_FUSE     0 auto | 1..4 = diffusion iterations fused per launch (tiled kernels)
+ *   IDG_OPT_ZCHUNK   0 auto | >0  = planes per CTA along z (tiled kernels)
  * idg_get_option returns the current value, or IDG_ERR_OPTION.
  */
 enum { IDG_OPT_KERNEL = 0, IDG_OPT_FUSE = 1, IDG_OPT_ZCHUNK = 2, IDG_OPT_COUNT_ = 3 };

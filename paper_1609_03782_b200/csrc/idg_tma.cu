@@ -1,0 +1,407 @@
+// TMA-pipelined, temporally fused IDG kernel (the fast path; steps a1-a6 of DESIGN.md section 7).
+//
+// Same decomposition as idg_tiled.cu -- a CTA owns a 128 x (WARPS*R) xy tile and streams along
+// z; a thread owns a float4 column of an R-row strip; x neighbours by warp shuffle, y
+// neighbours in registers with strip edges through shared memory, z neighbours in registers --
+// but level-0 planes are brought in by the Tensor Memory Accelerator: one elected thread issues
+// cp.async.bulk.tensor (3-D/4-D box 128 x TILE_Y x 1) into a ring of NS shared-memory stages,
+// NS-2 planes ahead of the plane being consumed, completion signalled on mbarriers.  The
+// per-level z rings are rotated by unrolling the plane loop three times (register renaming
+// instead of moves).
+//
+// Boundary (reading R1): TMA zero-fills outside the cube, so each thread whose cell lies just
+// outside a cube face reads the even-reflected cell instead (and writes it back to its own
+// cell for its neighbours); z reflection is done by the TMA plane coordinate.  The update is
+// symmetric under the reflection, so all fused levels satisfy the zero-flux replicate condition
+// bit for bit without any predicate in the arithmetic (see idg_tiled.cu).
+#include <cuda.h>
+
+#include <type_traits>
+
+#include "idg_kernels.cuh"
+
+namespace idg {
+
+namespace {
+
+constexpr int kLanes = 32;
+constexpr int kValidLanes = 30;
+constexpr int kTileX = 128;
+
+struct F4 { float x, y, z, w; };
+
+__device__ __forceinline__ F4 lds4(const float *p)
+{
+    const float4 v = *reinterpret_cast<const float4 *>(p);
+    return F4{v.x, v.y, v.z, v.w};
+}
+__device__ __forceinline__ void sts4(float *p, const F4 &a)
+{
+    *reinterpret_cast<float4 *>(p) = make_float4(a.x, a.y, a.z, a.w);
+}
+
+__device__ __forceinline__ F4 update4(const F4 &c, float left, float right, const F4 &ym, const F4 &yp,
+                                      const F4 &zm, const F4 &zp, const CubeParams &p)
+{
+    F4 o;
+    o.x = update(c.x, left, c.y, ym.x, yp.x, zm.x, zp.x, p.ax, p.ay, p.az, p.s);
+    o.y = update(c.y, c.x, c.z, ym.y, yp.y, zm.y, zp.y, p.ax, p.ay, p.az, p.s);
+    o.z = update(c.z, c.y, c.w, ym.z, yp.z, zm.z, zp.z, p.ax, p.ay, p.az, p.s);
+    o.w = update(c.w, c.z, right, ym.w, yp.w, zm.w, zp.w, p.ax, p.ay, p.az, p.s);
+    return o;
+}
+
+__device__ __forceinline__ int mirror(int i, int n)
+{
+    const int p = 2 * n;
+    int m = i % p;
+    if (m < 0) m += p;
+    return m < n ? m : p - 1 - m;
+}
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+// 4-D box load (x, y, z, cube) -> shared memory, completion on `bar`.
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, uint64_t *bar, int x, int y,
+                                            int z, int b)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z), "r"(b)
+        : "memory");
+}
+
+struct TmaArgs {
+    int tiles_x, tiles_y;
+    int zchunk;
+    int halo;
+};
+
+struct Maps {
+    CUtensorMap in, out, scratch;      // the three cubes (batch as 4th dimension) a launch may read
+};
+
+template <int T, int R, int WARPS, int NS>
+struct Smem {
+    static constexpr int TILE_Y = WARPS * R;
+    static constexpr int kStageFloats = TILE_Y * kTileX;
+    static constexpr size_t kStageBytes = (size_t)kStageFloats * sizeof(float);
+    static constexpr size_t kEdgeBytes = (size_t)(T > 1 ? T - 1 : 0) * 2 * WARPS * 2 * kLanes * sizeof(float4);
+    static constexpr size_t kBarOff = NS * kStageBytes + kEdgeBytes;
+    static constexpr size_t kBytes = kBarOff + NS * sizeof(uint64_t);
+};
+
+template <int TL, int R, int WARPS, int NS, int TMAX>
+__device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restrict__ dst, const Launch &L,
+                                         const TmaArgs &A, const CubeParams &prm, int b,
+                                         unsigned char *smem)
+{
+    using S = Smem<TMAX, R, WARPS, NS>;
+    constexpr int TILE_Y = WARPS * R;
+    float *stage0 = reinterpret_cast<float *>(smem);
+    float4 *edge = reinterpret_cast<float4 *>(smem + NS * S::kStageBytes);
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + S::kBarOff);
+
+    const int lane = threadIdx.x & 31;
+    const int wy = threadIdx.x >> 5;
+    const int nx4 = L.nx >> 2;
+    const int vy = TILE_Y - 2 * A.halo;
+    const int ti = blockIdx.x % A.tiles_x, tj = blockIdx.x / A.tiles_x;
+    const int tx0 = (ti * kValidLanes - 1) * 4;          // cube x of tile column 0
+    const int ty0 = tj * vy - A.halo;                    // cube y of tile row 0
+    const int x4 = ti * kValidLanes - 1 + lane;
+    const int row0 = wy * R;
+    const int z0 = blockIdx.y * A.zchunk;
+    const int z1 = min(z0 + A.zchunk, L.nz);
+    const int q_first = z0 - TL, q_last = z1 - 1 + TL;
+
+    // own cells, reflected source cells for positions just outside a cube face, store mask
+    int cell[R], scell[R];
+    unsigned ok = 0, fix = 0;
+    bool rev = false;
+    int slane = lane;
+    if (x4 < 0) { slane = lane + (-1 - x4) - x4; rev = true; }                 // x4' = -1 - x4
+    else if (x4 >= nx4) { slane = lane + (2 * nx4 - 1 - x4) - x4; rev = true; }
+    if (slane < 0 || slane >= kLanes) { slane = lane; rev = false; }            // beyond one reflection: unused cell
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int row = row0 + r, gy = ty0 + row;
+        cell[r] = row * kTileX + lane * 4;
+        int srow = row;
+        if (gy < 0) srow = (-1 - gy) - ty0;
+        else if (gy >= L.ny) srow = (2 * L.ny - 1 - gy) - ty0;
+        if (srow < 0 || srow >= TILE_Y) srow = row;
+        scell[r] = srow * kTileX + slane * 4;
+        if (scell[r] != cell[r]) fix |= 1u << r;
+        if (lane >= 1 && lane <= kValidLanes && x4 < nx4 && row >= A.halo && row < TILE_Y - A.halo &&
+            gy < L.ny)
+            ok |= 1u << r;
+    }
+    const int up_cell = max(row0 - 1, 0) * kTileX + lane * 4;              // level-0 strip-edge rows
+    const int dn_cell = min(row0 + R, TILE_Y - 1) * kTileX + lane * 4;
+    const int wy_up = max(wy - 1, 0), wy_dn = min(wy + 1, WARPS - 1);
+
+    const size_t plane = (size_t)L.nx * (size_t)L.ny;
+    float *po = dst + (long long)(ty0 + row0) * L.nx + (long long)x4 * 4 + (long long)(q_first - TL - 1) * (long long)plane;
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    auto issue = [&](int q) {       // thread 0: plane q -> stage (q - q_first) % NS
+        const int s = (q - q_first) % NS;
+        mbar_expect_tx(&full[s], (uint32_t)S::kStageBytes);
+        tma_load_4d(stage0 + (size_t)s * S::kStageFloats, map, &full[s], tx0, ty0, mirror(q, L.nz), b);
+    };
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int i = 0; i < NS - 2; ++i)
+            if (q_first + i <= q_last) issue(q_first + i);
+    }
+
+    F4 ring[3][TL][R];
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int t = 0; t < TL; ++t)
+#pragma unroll
+            for (int r = 0; r < R; ++r) ring[a][t][r] = F4{0.f, 0.f, 0.f, 0.f};
+
+    int q = q_first;
+    int par = 0;
+
+    // One plane step; P = rotation phase of the register rings (compile time).
+    auto step = [&](auto Pc) {
+        constexpr int P = decltype(Pc)::value;
+        F4(&zm)[TL][R] = ring[P % 3];
+        F4(&cc)[TL][R] = ring[(P + 1) % 3];
+        F4(&nw)[TL][R] = ring[(P + 2) % 3];
+
+        const unsigned it = (unsigned)(q - q_first);
+        const unsigned s = it % NS;
+        if (threadIdx.x == 0 && q + NS - 2 <= q_last) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            issue(q + NS - 2);                              // its stage held plane q-2: free since last barrier
+        }
+        const float *st = stage0 + (size_t)s * S::kStageFloats;                      // plane q
+        const float *stp = stage0 + (size_t)((it + NS - 1) % NS) * S::kStageFloats;  // plane q-1
+        mbar_wait(&full[s], (uint32_t)((it / NS) & 1));
+
+        // level-0 plane q: own cells (reflected source just outside a cube face)
+#pragma unroll
+        for (int r = 0; r < R; ++r) nw[0][r] = lds4(st + scell[r]);
+        if (fix) {
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+                if (fix & (1u << r)) {
+                    if (rev) nw[0][r] = F4{nw[0][r].w, nw[0][r].z, nw[0][r].y, nw[0][r].x};
+                    sts4(const_cast<float *>(st) + cell[r], nw[0][r]);
+                }
+        }
+        F4 out[R];
+#pragma unroll
+        for (int t = 0; t < TL; ++t) {
+            F4 up, dn;
+            if (t == 0) {
+                up = lds4(stp + up_cell);
+                dn = lds4(stp + dn_cell);
+            } else {
+                float4 *e_rd = edge + (((t - 1) * 2 + par) * WARPS) * 2 * kLanes;
+                float4 *e_wr = edge + (((t - 1) * 2 + (par ^ 1)) * WARPS) * 2 * kLanes;
+                e_wr[(wy * 2 + 0) * kLanes + lane] = make_float4(nw[t][0].x, nw[t][0].y, nw[t][0].z, nw[t][0].w);
+                e_wr[(wy * 2 + 1) * kLanes + lane] =
+                    make_float4(nw[t][R - 1].x, nw[t][R - 1].y, nw[t][R - 1].z, nw[t][R - 1].w);
+                const float4 u = e_rd[(wy_up * 2 + 1) * kLanes + lane];
+                const float4 d = e_rd[(wy_dn * 2 + 0) * kLanes + lane];
+                up = F4{u.x, u.y, u.z, u.w};
+                dn = F4{d.x, d.y, d.z, d.w};
+            }
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const F4 &c = cc[t][r];
+                const float left = __shfl_up_sync(0xffffffffu, c.w, 1);
+                const float right = __shfl_down_sync(0xffffffffu, c.x, 1);
+                const F4 &ym = (r == 0) ? up : cc[t][r - 1];
+                const F4 &yp = (r == R - 1) ? dn : cc[t][r + 1];
+                const F4 o = update4(c, left, right, ym, yp, zm[t][r], nw[t][r], prm);
+                if (t + 1 < TL) nw[t + 1][r] = o;
+                else out[r] = o;
+            }
+        }
+        // out = level-TL plane (q - TL)
+        po += plane;
+        const int zo = q - TL;
+        if (zo >= z0 && zo < z1) {
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+                if (ok & (1u << r))
+                    *reinterpret_cast<float4 *>(po + (long long)r * L.nx) =
+                        make_float4(out[r].x, out[r].y, out[r].z, out[r].w);
+        }
+        par ^= 1;
+        ++q;
+        __syncthreads();
+    };
+
+    while (true) {
+        step(std::integral_constant<int, 0>{});
+        if (q > q_last) break;
+        step(std::integral_constant<int, 1>{});
+        if (q > q_last) break;
+        step(std::integral_constant<int, 2>{});
+        if (q > q_last) break;
+    }
+}
+
+template <int T, int R, int WARPS, int NS>
+__global__ void __launch_bounds__(WARPS * 32, 1)
+idg_tma_kernel(const __grid_constant__ Launch L, const __grid_constant__ TmaArgs A,
+               const __grid_constant__ Maps M)
+{
+    extern __shared__ __align__(1024) unsigned char smem[];
+    const int b = blockIdx.z;
+    const CubeParams prm = cube_params(L, b);
+    const float *src;
+    float *dst;
+    const int now = route(L, b, prm, src, dst);
+    if (now == 0) return;
+    const size_t off = (size_t)b * (size_t)L.nx * (size_t)L.ny * (size_t)L.nz;
+    const CUtensorMap *map = (src == L.scratch + off) ? &M.scratch : (src == L.out + off) ? &M.out : &M.in;
+    if (now == T) tma_body<T, R, WARPS, NS, T>(map, dst, L, A, prm, b, smem);
+    else if (T > 1 && now == 1) tma_body<1, R, WARPS, NS, T>(map, dst, L, A, prm, b, smem);
+    else if (T > 2 && now == 2) tma_body<(T > 2 ? 2 : 1), R, WARPS, NS, T>(map, dst, L, A, prm, b, smem);
+    else if (T > 3 && now == 3) tma_body<(T > 3 ? 3 : 1), R, WARPS, NS, T>(map, dst, L, A, prm, b, smem);
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+bool encode_map(CUtensorMap *m, const float *base, const Launch &L, int tile_y)
+{
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return false;
+    const cuuint64_t dims[4] = {(cuuint64_t)L.nx, (cuuint64_t)L.ny, (cuuint64_t)L.nz, (cuuint64_t)L.batch};
+    const cuuint64_t strides[3] = {(cuuint64_t)L.nx * 4, (cuuint64_t)L.nx * L.ny * 4,
+                                   (cuuint64_t)L.nx * L.ny * (cuuint64_t)L.nz * 4};
+    const cuuint32_t box[4] = {(cuuint32_t)kTileX, (cuuint32_t)tile_y, 1, 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void *)base, dims, strides, box, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+int pick_zchunk(int nz, long tiles, int T)
+{
+    long best_cost = -1;
+    int best = nz;
+    for (int nchunks = 1; nchunks <= nz; ++nchunks) {
+        const int zc = (nz + nchunks - 1) / nchunks;
+        const long ctas = tiles * ((nz + zc - 1) / zc);
+        const long waves = (ctas + 147) / 148;
+        const long cost = waves * (zc + 2 * T + 3);      // +3: prologue and pipeline fill, in plane-steps
+        if (best_cost < 0 || cost < best_cost) {
+            best_cost = cost;
+            best = zc;
+        }
+        if (zc == 1) break;
+    }
+    return best;
+}
+
+template <int T, int R, int WARPS, int NS>
+cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st)
+{
+    using S = Smem<T, R, WARPS, NS>;
+    constexpr int TILE_Y = WARPS * R;
+    static_assert(TILE_Y > 2 * T, "tile must be taller than its halo");
+    static_assert(S::kBytes <= 227 * 1024, "shared memory budget");
+    TmaArgs A;
+    A.halo = T;
+    A.tiles_x = (L.nx / 4 + kValidLanes - 1) / kValidLanes;
+    A.tiles_y = (L.ny + (TILE_Y - 2 * T) - 1) / (TILE_Y - 2 * T);
+    const long tiles = (long)A.tiles_x * A.tiles_y;
+    if (tiles > 0x7fffffffL) return cudaErrorInvalidValue;
+    A.zchunk = zchunk > 0 ? (zchunk < L.nz ? zchunk : L.nz) : pick_zchunk(L.nz, tiles * L.batch, T);
+    if ((L.nz + A.zchunk - 1) / A.zchunk > 65535) A.zchunk = (L.nz + 65534) / 65535;
+    Maps M;
+    if (!encode_map(&M.in, L.in, L, TILE_Y) || !encode_map(&M.out, L.out, L, TILE_Y) ||
+        !encode_map(&M.scratch, L.scratch, L, TILE_Y))
+        return cudaErrorNotSupported;
+    auto kern = idg_tma_kernel<T, R, WARPS, NS>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::kBytes);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    dim3 grid((unsigned)tiles, (unsigned)((L.nz + A.zchunk - 1) / A.zchunk), (unsigned)L.batch);
+    kern<<<grid, WARPS * 32, S::kBytes, st>>>(L, A, M);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+// The reflected source of a halo cell must lie inside the same tile: needs ny >= 4 (max halo)
+// and a usable driver entry point for tensor-map encoding.
+bool tma_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch)
+{
+    (void)nz;
+    if (nx % 4 != 0 || ny < 4) return false;
+    const uintptr_t m = (uintptr_t)in | (uintptr_t)out | (uintptr_t)scratch;
+    if ((m & 15u) != 0) return false;
+    return encode_fn() != nullptr;
+}
+
+cudaError_t launch_tma(const Launch &L, int zchunk, cudaStream_t st)
+{
+    switch (L.fuse) {
+    case 1: return launch_cfg<1, 4, 16, 4>(L, zchunk, st);
+    case 2: return launch_cfg<2, 4, 16, 4>(L, zchunk, st);
+    case 3: return launch_cfg<3, 4, 8, 4>(L, zchunk, st);
+    case 4: return launch_cfg<4, 4, 8, 4>(L, zchunk, st);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace idg

@@ -27,8 +27,9 @@ def B():
 
 
 # (kernel, fuse) plans every parity case runs under
-PLANS = [(1, 0), (2, 1), (2, 2), (2, 3), (2, 4), (0, 0)]
-PLAN_IDS = ["naive", "tiled-T1", "tiled-T2", "tiled-T3", "tiled-T4", "auto"]
+PLANS = [(1, 0), (2, 1), (2, 2), (2, 3), (2, 4), (3, 1), (3, 2), (3, 3), (3, 4), (0, 0)]
+PLAN_IDS = ["naive", "tiled-T1", "tiled-T2", "tiled-T3", "tiled-T4", "tma-T1", "tma-T2", "tma-T3", "tma-T4",
+            "auto"]
 
 
 def set_plan(B, plan, zchunk=0):
@@ -80,9 +81,10 @@ def test_config0_full_cube(B, oracle, plan):
 
 @pytest.mark.parametrize("zchunk", [1, 3, 16, 1000])
 @pytest.mark.parametrize("fuse", [1, 2, 4])
-def test_zchunk_variants(B, oracle, fuse, zchunk):
-    """z-chunking of the tiled kernel (ragged last chunk, chunk < T, chunk > nz)."""
-    set_plan(B, (2, fuse), zchunk)
+@pytest.mark.parametrize("kernel", [2, 3])
+def test_zchunk_variants(B, oracle, kernel, fuse, zchunk):
+    """z-chunking of the tiled kernels (ragged last chunk, chunk < T, chunk > nz)."""
+    set_plan(B, (kernel, fuse), zchunk)
     rng = np.random.default_rng(5)
     a = rng.normal(0, 2, (19, 70, 136)).astype(np.float32)
     p = B.Params(K=2.0, tau=0.03, cx=5.0, cy=5.0, cz=5.0, rms=2.0)
@@ -311,6 +313,7 @@ def test_launch_count(B):
     t = torch.zeros(4, 8, 8, device="cuda")
     B.idg_filter(t, 7)
     assert B.idg_last_launch_count() == 7
-    set_plan(B, (2, 2))
-    B.idg_filter(t, 7)
-    assert B.idg_last_launch_count() == 4
+    for k in (2, 3):
+        set_plan(B, (k, 2))
+        B.idg_filter(t, 7)
+        assert B.idg_last_launch_count() == 4
