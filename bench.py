@@ -193,6 +193,7 @@ def run_ours(args) -> None:
     B.lib()                                   # fail loudly if the extension is missing
     B.idg_set_option(B.IDG_OPT_FUSE, args.fuse)
     B.idg_set_option(B.IDG_OPT_ZCHUNK, args.zchunk)
+    B.idg_set_option(B.IDG_OPT_TILE, args.tile)
 
     threads = max(1, (os.cpu_count() or 1) // max(1, world))
     cube, n = make_cube(args.workload, seed_offset=rank, threads=threads)
@@ -303,6 +304,7 @@ def main() -> None:
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--fuse", type=int, default=0, help="iterations fused per launch (0 = library default)")
     ap.add_argument("--zchunk", type=int, default=0, help="planes per CTA along z (0 = library default)")
+    ap.add_argument("--tile", type=int, default=0, help="TMA kernel tile variant (0 = library default)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -11,7 +11,7 @@
 
 namespace {
 
-int g_opt[IDG_OPT_COUNT_] = {0, 0, 0};
+int g_opt[IDG_OPT_COUNT_] = {0, 0, 0, 0};
 thread_local int t_launches = 0;
 
 constexpr size_t kAlign = 256;
@@ -145,7 +145,7 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     }
     for (int done = 0; done < max_n; done += fuse) {
         L.iter_done = done;
-        e = (kernel == 3)   ? idg::launch_tma(L, g_opt[IDG_OPT_ZCHUNK], st)
+        e = (kernel == 3)   ? idg::launch_tma(L, g_opt[IDG_OPT_ZCHUNK], g_opt[IDG_OPT_TILE], st)
             : (kernel == 2) ? idg::launch_tiled(L, g_opt[IDG_OPT_ZCHUNK], st)
                             : idg::launch_naive(L, st);
         if (e != cudaSuccess) return (int)e;
@@ -273,6 +273,7 @@ int idg_set_option(int key, int value)
     if (key == IDG_OPT_KERNEL && (value < 0 || value > 3)) return IDG_ERR_OPTION;
     if (key == IDG_OPT_FUSE && (value < 0 || value > 4)) return IDG_ERR_OPTION;
     if (key == IDG_OPT_ZCHUNK && value < 0) return IDG_ERR_OPTION;
+    if (key == IDG_OPT_TILE && (value < 0 || value > 2)) return IDG_ERR_OPTION;
     g_opt[key] = value;
     return IDG_OK;
 }

@@ -81,7 +81,7 @@ __device__ __forceinline__ float update(float c, float xm, float xp, float ym, f
 cudaError_t launch_naive(const Launch &L, cudaStream_t st);
 cudaError_t launch_tiled(const Launch &L, int zchunk, cudaStream_t st);
 bool tiled_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
-cudaError_t launch_tma(const Launch &L, int zchunk, cudaStream_t st);
+cudaError_t launch_tma(const Launch &L, int zchunk, int tile, cudaStream_t st);
 bool tma_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
 
 }  // namespace idg

@@ -40,15 +40,52 @@ __device__ __forceinline__ void sts4(float *p, const F4 &a)
     *reinterpret_cast<float4 *>(p) = make_float4(a.x, a.y, a.z, a.w);
 }
 
-__device__ __forceinline__ F4 update4(const F4 &c, float left, float right, const F4 &ym, const F4 &yp,
-                                      const F4 &zm, const F4 &zp, const CubeParams &p)
+// Four voxel updates (Eq. 7) of one float4 column with packed fp32x2 arithmetic (FFMA2 / FADD2 /
+// FMUL2: two IEEE fp32 results per issued instruction; each component rounds exactly like the
+// scalar update() of idg_kernels.cuh, so results are bit-identical to the scalar kernels).
+struct Consts {
+    float2 m2, ax, ay, az, s, one;
+};
+__device__ __forceinline__ Consts make_consts(const CubeParams &p)
 {
-    F4 o;
-    o.x = update(c.x, left, c.y, ym.x, yp.x, zm.x, zp.x, p.ax, p.ay, p.az, p.s);
-    o.y = update(c.y, c.x, c.z, ym.y, yp.y, zm.y, zp.y, p.ax, p.ay, p.az, p.s);
-    o.z = update(c.z, c.y, c.w, ym.z, yp.z, zm.z, zp.z, p.ax, p.ay, p.az, p.s);
-    o.w = update(c.w, c.z, right, ym.w, yp.w, zm.w, zp.w, p.ax, p.ay, p.az, p.s);
-    return o;
+    Consts k;
+    k.m2 = make_float2(-2.0f, -2.0f);
+    k.ax = make_float2(p.ax, p.ax);
+    k.ay = make_float2(p.ay, p.ay);
+    k.az = make_float2(p.az, p.az);
+    k.s = make_float2(p.s, p.s);
+    k.one = make_float2(1.0f, 1.0f);
+    return k;
+}
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float2 update2(float2 c, float2 sx, float2 ym, float2 yp, float2 zm, float2 zp,
+                                          const Consts &k)
+{
+    const float2 dx = __ffma2_rn(k.m2, c, sx);
+    const float2 dy = __ffma2_rn(k.m2, c, __fadd2_rn(yp, ym));
+    const float2 dz = __ffma2_rn(k.m2, c, __fadd2_rn(zp, zm));
+    const float2 lap = __ffma2_rn(k.az, dz, __ffma2_rn(k.ay, dy, __fmul2_rn(k.ax, dx)));
+    const float2 u = __fmul2_rn(c, k.s);
+    const float2 den = __ffma2_rn(u, u, k.one);
+    const float2 r = make_float2(rcp_approx(den.x), rcp_approx(den.y));
+    return __ffma2_rn(lap, r, c);
+}
+__device__ __forceinline__ F4 update4(const F4 &c, float left, float right, const F4 &ym, const F4 &yp,
+                                      const F4 &zm, const F4 &zp, const Consts &k)
+{
+    // x neighbour sums stay scalar: their operands straddle the register pairs
+    const float2 sx01 = make_float2(c.y + left, c.z + c.x);
+    const float2 sx23 = make_float2(c.w + c.y, right + c.z);
+    const float2 o01 = update2(make_float2(c.x, c.y), sx01, make_float2(ym.x, ym.y), make_float2(yp.x, yp.y),
+                               make_float2(zm.x, zm.y), make_float2(zp.x, zp.y), k);
+    const float2 o23 = update2(make_float2(c.z, c.w), sx23, make_float2(ym.z, ym.w), make_float2(yp.z, yp.w),
+                               make_float2(zm.z, zm.w), make_float2(zp.z, zp.w), k);
+    return F4{o01.x, o01.y, o23.x, o23.y};
 }
 
 __device__ __forceinline__ int mirror(int i, int n)
@@ -183,6 +220,7 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
             if (q_first + i <= q_last) issue(q_first + i);
     }
 
+    const Consts kc = make_consts(prm);
     F4 ring[3][TL][R];
 #pragma unroll
     for (int a = 0; a < 3; ++a)
@@ -247,7 +285,7 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
                 const float right = __shfl_down_sync(0xffffffffu, c.x, 1);
                 const F4 &ym = (r == 0) ? up : cc[t][r - 1];
                 const F4 &yp = (r == R - 1) ? dn : cc[t][r + 1];
-                const F4 o = update4(c, left, right, ym, yp, zm[t][r], nw[t][r], prm);
+                const F4 o = update4(c, left, right, ym, yp, zm[t][r], nw[t][r], kc);
                 if (t + 1 < TL) nw[t + 1][r] = o;
                 else out[r] = o;
             }
@@ -277,8 +315,8 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
     }
 }
 
-template <int T, int R, int WARPS, int NS>
-__global__ void __launch_bounds__(WARPS * 32, 1)
+template <int T, int R, int WARPS, int NS, int MINB>
+__global__ void __launch_bounds__(WARPS * 32, MINB)
 idg_tma_kernel(const __grid_constant__ Launch L, const __grid_constant__ TmaArgs A,
                const __grid_constant__ Maps M)
 {
@@ -331,14 +369,14 @@ bool encode_map(CUtensorMap *m, const float *base, const Launch &L, int tile_y)
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-int pick_zchunk(int nz, long tiles, int T)
+int pick_zchunk(int nz, long tiles, int T, int slots)
 {
     long best_cost = -1;
     int best = nz;
     for (int nchunks = 1; nchunks <= nz; ++nchunks) {
         const int zc = (nz + nchunks - 1) / nchunks;
         const long ctas = tiles * ((nz + zc - 1) / zc);
-        const long waves = (ctas + 147) / 148;
+        const long waves = (ctas + slots - 1) / slots;
         const long cost = waves * (zc + 2 * T + 3);      // +3: prologue and pipeline fill, in plane-steps
         if (best_cost < 0 || cost < best_cost) {
             best_cost = cost;
@@ -349,26 +387,26 @@ int pick_zchunk(int nz, long tiles, int T)
     return best;
 }
 
-template <int T, int R, int WARPS, int NS>
+template <int T, int R, int WARPS, int NS, int MINB>
 cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st)
 {
     using S = Smem<T, R, WARPS, NS>;
     constexpr int TILE_Y = WARPS * R;
     static_assert(TILE_Y > 2 * T, "tile must be taller than its halo");
-    static_assert(S::kBytes <= 227 * 1024, "shared memory budget");
+    static_assert(S::kBytes * MINB <= 227 * 1024, "shared memory budget");
     TmaArgs A;
     A.halo = T;
     A.tiles_x = (L.nx / 4 + kValidLanes - 1) / kValidLanes;
     A.tiles_y = (L.ny + (TILE_Y - 2 * T) - 1) / (TILE_Y - 2 * T);
     const long tiles = (long)A.tiles_x * A.tiles_y;
     if (tiles > 0x7fffffffL) return cudaErrorInvalidValue;
-    A.zchunk = zchunk > 0 ? (zchunk < L.nz ? zchunk : L.nz) : pick_zchunk(L.nz, tiles * L.batch, T);
+    A.zchunk = zchunk > 0 ? (zchunk < L.nz ? zchunk : L.nz) : pick_zchunk(L.nz, tiles * L.batch, T, 148 * MINB);
     if ((L.nz + A.zchunk - 1) / A.zchunk > 65535) A.zchunk = (L.nz + 65534) / 65535;
     Maps M;
     if (!encode_map(&M.in, L.in, L, TILE_Y) || !encode_map(&M.out, L.out, L, TILE_Y) ||
         !encode_map(&M.scratch, L.scratch, L, TILE_Y))
         return cudaErrorNotSupported;
-    auto kern = idg_tma_kernel<T, R, WARPS, NS>;
+    auto kern = idg_tma_kernel<T, R, WARPS, NS, MINB>;
     static bool attr_done = false;
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::kBytes);
@@ -393,13 +431,16 @@ bool tma_supported(int nx, int ny, int nz, const void *in, const void *out, cons
     return encode_fn() != nullptr;
 }
 
-cudaError_t launch_tma(const Launch &L, int zchunk, cudaStream_t st)
+// tile: 0 auto | 1 = 128x64 tile, 512 threads, one CTA per SM | 2 = 128x32 tile, 256 threads,
+// two CTAs per SM (T <= 2; deeper fusion needs the registers of a lone CTA)
+cudaError_t launch_tma(const Launch &L, int zchunk, int tile, cudaStream_t st)
 {
+    const bool small = (tile == 2);
     switch (L.fuse) {
-    case 1: return launch_cfg<1, 4, 16, 4>(L, zchunk, st);
-    case 2: return launch_cfg<2, 4, 16, 4>(L, zchunk, st);
-    case 3: return launch_cfg<3, 4, 8, 4>(L, zchunk, st);
-    case 4: return launch_cfg<4, 4, 8, 4>(L, zchunk, st);
+    case 1: return small ? launch_cfg<1, 4, 8, 4, 2>(L, zchunk, st) : launch_cfg<1, 4, 16, 4, 1>(L, zchunk, st);
+    case 2: return small ? launch_cfg<2, 4, 8, 4, 2>(L, zchunk, st) : launch_cfg<2, 4, 16, 4, 1>(L, zchunk, st);
+    case 3: return launch_cfg<3, 4, 8, 4, 1>(L, zchunk, st);
+    case 4: return launch_cfg<4, 4, 8, 4, 1>(L, zchunk, st);
     default: return cudaErrorInvalidValue;
     }
 }

@@ -22,7 +22,7 @@ def B():
     from paper_1609_03782_b200 import binding
     binding.lib()           # fails loudly if the extension is missing
     yield binding
-    for k in (binding.IDG_OPT_KERNEL, binding.IDG_OPT_FUSE, binding.IDG_OPT_ZCHUNK):
+    for k in (binding.IDG_OPT_KERNEL, binding.IDG_OPT_FUSE, binding.IDG_OPT_ZCHUNK, binding.IDG_OPT_TILE):
         binding.idg_set_option(k, 0)
 
 
@@ -32,10 +32,11 @@ PLAN_IDS = ["naive", "tiled-T1", "tiled-T2", "tiled-T3", "tiled-T4", "tma-T1", "
             "auto"]
 
 
-def set_plan(B, plan, zchunk=0):
+def set_plan(B, plan, zchunk=0, tile=0):
     B.idg_set_option(B.IDG_OPT_KERNEL, plan[0])
     B.idg_set_option(B.IDG_OPT_FUSE, plan[1])
     B.idg_set_option(B.IDG_OPT_ZCHUNK, zchunk)
+    B.idg_set_option(B.IDG_OPT_TILE, tile)
 
 
 def gpu(B, cube_np, n, p, **kw):
@@ -90,6 +91,22 @@ def test_zchunk_variants(B, oracle, kernel, fuse, zchunk):
     p = B.Params(K=2.0, tau=0.03, cx=5.0, cy=5.0, cz=5.0, rms=2.0)
     ref = oracle.idg_filter_oracle(a, 7, **p.f32())
     assert err(gpu(B, a, 7, p), ref, 2.0) <= TOL
+
+
+@pytest.mark.parametrize("tile", [1, 2])
+@pytest.mark.parametrize("fuse", [1, 2, 4])
+def test_tma_tile_variants(B, oracle, fuse, tile):
+    """Both tilings of the TMA kernel (128x64 one CTA/SM, 128x32 two CTAs/SM) on a cube spanning
+    several tiles in x and y with ragged tails, and on the config-0 cube."""
+    from paper_1609_03782_b200 import synth
+    set_plan(B, (3, fuse), 0, tile)
+    rng = np.random.default_rng(17)
+    a = rng.normal(0, 2, (11, 150, 268)).astype(np.float32)
+    p = B.Params(K=1.0, tau=0.03, cx=4.0, cy=5.0, cz=6.0, rms=2.0)
+    assert err(gpu(B, a, 6, p), oracle.idg_filter_oracle(a, 6, **p.f32()), 2.0) <= TOL
+    c = synth.modelb_like(seed=1000, snr=32.0)
+    p = B.Params()
+    assert err(gpu(B, c.data, 10, p), oracle.idg_filter_oracle(c.data, 10, **p.f32()), c.rms) <= TOL
 
 
 def test_config1_parameter_sweep(B, oracle):
