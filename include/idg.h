@@ -132,14 +132,17 @@ int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
 /*
  * Process-wide tuning knobs (tests and benchmarks; defaults give the fastest plan).
  *   IDG_OPT_KERNEL   0 auto | 1 naive (one thread per voxel) | 2 tiled z-streaming kernel (global loads)
- *                    | 3 tiled z-streaming kernel fed by TMA (the fast path)
+ *                    | 3 tiled z-streaming kernel fed by TMA | 4 persistent warp-decoupled TMA kernel
+ *                    (the fast path)
  *   IDG_OPT_FUSE     0 auto | 1..4 = diffusion iterations fused per launch (tiled kernels)
  *   IDG_OPT_ZCHUNK   0 auto | >0  = planes per CTA along z (tiled kernels)
  *   IDG_OPT_TILE     0 auto | 1 = 128x64 tile, one 512-thread CTA per SM | 2 = 128x32 tile, two
- *                    256-thread CTAs per SM (TMA kernel, fuse <= 2)
+ *                    256-thread CTAs per SM (TMA kernels, fuse <= 2)
+ *   IDG_OPT_CTAS     0 auto | >0  = persistent grid size of kernel 4
  * idg_get_option returns the current value, or IDG_ERR_OPTION.
  */
-enum { IDG_OPT_KERNEL = 0, IDG_OPT_FUSE = 1, IDG_OPT_ZCHUNK = 2, IDG_OPT_TILE = 3, IDG_OPT_COUNT_ = 4 };
+enum { IDG_OPT_KERNEL = 0, IDG_OPT_FUSE = 1, IDG_OPT_ZCHUNK = 2, IDG_OPT_TILE = 3, IDG_OPT_CTAS = 4,
+       IDG_OPT_COUNT_ = 5 };
 int idg_set_option(int key, int value);
 int idg_get_option(int key);
 

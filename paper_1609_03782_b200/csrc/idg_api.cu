@@ -11,7 +11,7 @@
 
 namespace {
 
-int g_opt[IDG_OPT_COUNT_] = {0, 0, 0, 0};
+int g_opt[IDG_OPT_COUNT_] = {0, 0, 0, 0, 0};
 thread_local int t_launches = 0;
 
 constexpr size_t kAlign = 256;
@@ -88,7 +88,9 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     const bool can_tile = idg::tiled_supported(nx, ny, nz, cubes, out, scratch);
     const bool can_tma = idg::tma_supported(nx, ny, nz, cubes, out, scratch);
     int kernel = g_opt[IDG_OPT_KERNEL];
+    const bool can_stream = idg::stream_supported(nx, ny, nz, cubes, out, scratch);
     if (kernel == 0) kernel = can_tma ? 3 : (can_tile ? 2 : 1);
+    if (kernel == 4 && !can_stream) kernel = 2;
     if (kernel == 3 && !can_tma) kernel = 2;
     if (kernel == 2 && !can_tile) kernel = 1;
     int fuse = 1;
@@ -145,7 +147,8 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     }
     for (int done = 0; done < max_n; done += fuse) {
         L.iter_done = done;
-        e = (kernel == 3)   ? idg::launch_tma(L, g_opt[IDG_OPT_ZCHUNK], g_opt[IDG_OPT_TILE], st)
+        e = (kernel == 4)   ? idg::launch_stream(L, g_opt[IDG_OPT_CTAS], g_opt[IDG_OPT_TILE], st)
+            : (kernel == 3) ? idg::launch_tma(L, g_opt[IDG_OPT_ZCHUNK], g_opt[IDG_OPT_TILE], st)
             : (kernel == 2) ? idg::launch_tiled(L, g_opt[IDG_OPT_ZCHUNK], st)
                             : idg::launch_naive(L, st);
         if (e != cudaSuccess) return (int)e;
@@ -270,10 +273,11 @@ int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
 int idg_set_option(int key, int value)
 {
     if (key < 0 || key >= IDG_OPT_COUNT_) return IDG_ERR_OPTION;
-    if (key == IDG_OPT_KERNEL && (value < 0 || value > 3)) return IDG_ERR_OPTION;
+    if (key == IDG_OPT_KERNEL && (value < 0 || value > 4)) return IDG_ERR_OPTION;
     if (key == IDG_OPT_FUSE && (value < 0 || value > 4)) return IDG_ERR_OPTION;
     if (key == IDG_OPT_ZCHUNK && value < 0) return IDG_ERR_OPTION;
     if (key == IDG_OPT_TILE && (value < 0 || value > 2)) return IDG_ERR_OPTION;
+    if (key == IDG_OPT_CTAS && value < 0) return IDG_ERR_OPTION;
     g_opt[key] = value;
     return IDG_OK;
 }

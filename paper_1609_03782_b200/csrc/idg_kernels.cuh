@@ -83,5 +83,7 @@ cudaError_t launch_tiled(const Launch &L, int zchunk, cudaStream_t st);
 bool tiled_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
 cudaError_t launch_tma(const Launch &L, int zchunk, int tile, cudaStream_t st);
 bool tma_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
+cudaError_t launch_stream(const Launch &L, int nctas, int tile, cudaStream_t st);
+bool stream_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
 
 }  // namespace idg

@@ -22,21 +22,24 @@ def B():
     from paper_1609_03782_b200 import binding
     binding.lib()           # fails loudly if the extension is missing
     yield binding
-    for k in (binding.IDG_OPT_KERNEL, binding.IDG_OPT_FUSE, binding.IDG_OPT_ZCHUNK, binding.IDG_OPT_TILE):
+    for k in (binding.IDG_OPT_KERNEL, binding.IDG_OPT_FUSE, binding.IDG_OPT_ZCHUNK, binding.IDG_OPT_TILE,
+              binding.IDG_OPT_CTAS):
         binding.idg_set_option(k, 0)
 
 
 # (kernel, fuse) plans every parity case runs under
-PLANS = [(1, 0), (2, 1), (2, 2), (2, 3), (2, 4), (3, 1), (3, 2), (3, 3), (3, 4), (0, 0)]
+PLANS = [(1, 0), (2, 1), (2, 2), (2, 3), (2, 4), (3, 1), (3, 2), (3, 3), (3, 4),
+         (4, 1), (4, 2), (4, 3), (4, 4), (0, 0)]
 PLAN_IDS = ["naive", "tiled-T1", "tiled-T2", "tiled-T3", "tiled-T4", "tma-T1", "tma-T2", "tma-T3", "tma-T4",
-            "auto"]
+            "stream-T1", "stream-T2", "stream-T3", "stream-T4", "auto"]
 
 
-def set_plan(B, plan, zchunk=0, tile=0):
+def set_plan(B, plan, zchunk=0, tile=0, ctas=0):
     B.idg_set_option(B.IDG_OPT_KERNEL, plan[0])
     B.idg_set_option(B.IDG_OPT_FUSE, plan[1])
     B.idg_set_option(B.IDG_OPT_ZCHUNK, zchunk)
     B.idg_set_option(B.IDG_OPT_TILE, tile)
+    B.idg_set_option(B.IDG_OPT_CTAS, ctas)
 
 
 def gpu(B, cube_np, n, p, **kw):
@@ -107,6 +110,19 @@ def test_tma_tile_variants(B, oracle, fuse, tile):
     c = synth.modelb_like(seed=1000, snr=32.0)
     p = B.Params()
     assert err(gpu(B, c.data, 10, p), oracle.idg_filter_oracle(c.data, 10, **p.f32()), c.rms) <= TOL
+
+
+@pytest.mark.parametrize("ctas", [1, 2, 7, 61, 148, 1000])
+@pytest.mark.parametrize("tile", [1, 2])
+@pytest.mark.parametrize("fuse", [1, 2, 3, 4])
+def test_stream_grid_variants(B, oracle, fuse, tile, ctas):
+    """Persistent kernel: any split of the tile-plane stream over CTAs (segments that start and end
+    mid-tile, one CTA walking over all tiles, more CTAs than planes) gives the same cube."""
+    set_plan(B, (4, fuse), 0, tile, ctas)
+    rng = np.random.default_rng(23)
+    a = rng.normal(0, 2, (13, 150, 268)).astype(np.float32)
+    p = B.Params(K=1.0, tau=0.03, cx=4.0, cy=5.0, cz=6.0, rms=2.0)
+    assert err(gpu(B, a, 7, p), oracle.idg_filter_oracle(a, 7, **p.f32()), 2.0) <= TOL
 
 
 def test_config1_parameter_sweep(B, oracle):
