@@ -72,6 +72,14 @@ __device__ __forceinline__ uint32_t atom_add_acq_rel(uint32_t addr, uint32_t v)
     asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(addr), "r"(v) : "memory");
     return old;
 }
+// relaxed counter: enough for handing back a buffer that was only READ (the loaded values have
+// been consumed by the time the counter is bumped), as with a consumer-release mbarrier arrive
+__device__ __forceinline__ uint32_t atom_add_relaxed(uint32_t addr, uint32_t v)
+{
+    uint32_t old;
+    asm volatile("atom.relaxed.cta.shared::cta.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(addr), "r"(v) : "memory");
+    return old;
+}
 __device__ __forceinline__ void sts32(uint32_t addr, uint32_t v)
 {
     asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
