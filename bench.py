@@ -218,6 +218,7 @@ def run_ours(args) -> None:
     for _ in range(max(3, args.warmup)):
         step()
     launches_per_step = B.idg_last_launch_count()
+    plan = B.idg_last_plan()
     fuse = -(-n // launches_per_step)
     barrier()
     sampler = ClockSampler(local)
@@ -266,7 +267,7 @@ def run_ours(args) -> None:
     peak, peak_src = measured_peak_gbs()
     ms_launch = ms_step / launches_per_step
     achieved = BYTES_PER_VOXEL_ITER * N * fuse / (ms_launch * 1e-3) / 1e9     # algorithmic GB/s per launch
-    kernel_tag = f"idg_tiled_T{fuse}_{args.workload}"
+    kernel_tag = f"{plan} {args.workload}"
     cpu_v, cores, sample, _ = oracle_rate(cube.data, n, 15.0, p.f32())
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -279,7 +280,7 @@ def run_ours(args) -> None:
                    "paper_context": "GTX860M OpenGL 0.90, i7 8 threads 0.036 Gvoxel-iter/s (PAPER.md:408-414)"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": ncu_traffic_bytes(kernel_tag),
-                     "kernel": f"idg_tiled_kernel<T={fuse}>", "ms_per_launch": ms_launch,
+                     "kernel": plan, "ms_per_launch": ms_launch,
                      "algorithmic_bytes_per_launch": BYTES_PER_VOXEL_ITER * N * fuse,
                      "peak_source": peak_src,
                      "note": "algorithmic bytes = 8 B x voxels x fused iterations (what an un-fused sweep must "

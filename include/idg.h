@@ -137,7 +137,7 @@ int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
  *   IDG_OPT_FUSE     0 auto | 1..4 = diffusion iterations fused per launch (tiled kernels)
  *   IDG_OPT_ZCHUNK   0 auto | >0  = planes per CTA along z (tiled kernels)
  *   IDG_OPT_TILE     0 auto | 1 = 128x64 tile, one 512-thread CTA per SM | 2 = 128x32 tile, two
- *                    256-thread CTAs per SM (TMA kernels, fuse <= 2)
+ *                    256-thread CTAs per SM | 3, 4 = further tilings of kernel 4 (see idg_stream.cu)
  *   IDG_OPT_CTAS     0 auto | >0  = persistent grid size of kernel 4
  * idg_get_option returns the current value, or IDG_ERR_OPTION.
  */
@@ -151,6 +151,12 @@ int idg_get_option(int key);
  * (for bench.py's "gpu_launches" claim).
  */
 int idg_last_launch_count(void);
+
+/*
+ * Plan of the last filter call on this thread: "<kernel name> fuse=<T> tile=<variant>" (static
+ * thread-local storage; for bench.py's roofline record).
+ */
+const char *idg_last_plan(void);
 
 #ifdef __cplusplus
 }

@@ -23,7 +23,7 @@ KERNEL_AUTO, KERNEL_NAIVE, KERNEL_TILED, KERNEL_TMA, KERNEL_STREAM = 0, 1, 2, 3,
 # every symbol include/idg.h declares (tests check the library exports them all)
 SYMBOLS = ("idg_version", "idg_status_string", "idg_params_check", "idg_workspace_bytes",
            "idg_filter", "idg_filter_ws", "idg_filter_batched", "idg_filter_host",
-           "idg_set_option", "idg_get_option", "idg_last_launch_count")
+           "idg_set_option", "idg_get_option", "idg_last_launch_count", "idg_last_plan")
 
 
 class IdgParams(ctypes.Structure):
@@ -89,6 +89,7 @@ def lib() -> ctypes.CDLL:
         L.idg_get_option.restype = i
         L.idg_get_option.argtypes = [i]
         L.idg_last_launch_count.restype = i
+        L.idg_last_plan.restype = ctypes.c_char_p
         _lib = L
     return _lib
 
@@ -137,6 +138,10 @@ def idg_get_option(key: int) -> int:
 
 def idg_last_launch_count() -> int:
     return int(lib().idg_last_launch_count())
+
+
+def idg_last_plan() -> str:
+    return lib().idg_last_plan().decode()
 
 
 def alloc_workspace(nx: int, ny: int, nz: int, batch: int = 1, device="cuda") -> torch.Tensor:

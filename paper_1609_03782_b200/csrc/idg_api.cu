@@ -2,6 +2,7 @@
 // validation, parameter preparation (step a0), launch planning.  Every voxel
 // update runs in the kernels of idg_naive.cu / idg_tiled.cu.
 #include <math.h>
+#include <stdio.h>
 #include <string.h>
 
 #include <vector>
@@ -13,6 +14,7 @@ namespace {
 
 int g_opt[IDG_OPT_COUNT_] = {0, 0, 0, 0, 0};
 thread_local int t_launches = 0;
+thread_local char t_plan[96] = "none";
 
 constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
@@ -87,16 +89,46 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     // Plan: kernel variant and iterations fused per launch.
     const bool can_tile = idg::tiled_supported(nx, ny, nz, cubes, out, scratch);
     const bool can_tma = idg::tma_supported(nx, ny, nz, cubes, out, scratch);
-    int kernel = g_opt[IDG_OPT_KERNEL];
     const bool can_stream = idg::stream_supported(nx, ny, nz, cubes, out, scratch);
-    if (kernel == 0) kernel = can_tma ? 3 : (can_tile ? 2 : 1);
+    int kernel = g_opt[IDG_OPT_KERNEL];
+    int fuse = g_opt[IDG_OPT_FUSE];
+    int tile = g_opt[IDG_OPT_TILE];
+    if (kernel == 0) {
+        // Measured on B200 (profiles/): batches and cubes of at most 128 columns run best on the persistent
+        // kernel (one tile column, no idle tail between cubes); large single cubes on the z-chunked TMA
+        // kernel with two CTAs per SM; cubes too small to fill the GPU want few, deeply fused launches.
+        const double work = (double)N * (double)batch;
+        if (can_stream && (batch > 1 || nx <= 128) && work >= 4.0e6) {
+            kernel = 4;
+            if (!fuse) fuse = 2;
+            if (!tile) tile = 2;
+        } else if (can_tma) {
+            kernel = 3;
+            if (work >= 1.6e7) {
+                if (!fuse) fuse = 2;
+                if (!tile) tile = 2;
+            } else if (!fuse) {
+                fuse = 3;
+            }
+        } else {
+            kernel = can_tile ? 2 : 1;
+        }
+    }
     if (kernel == 4 && !can_stream) kernel = 2;
     if (kernel == 3 && !can_tma) kernel = 2;
     if (kernel == 2 && !can_tile) kernel = 1;
-    int fuse = 1;
     if (kernel >= 2) {
-        fuse = g_opt[IDG_OPT_FUSE] ? g_opt[IDG_OPT_FUSE] : 2;
+        if (!fuse) fuse = 2;
         if (fuse > max_n && max_n > 0) fuse = max_n;
+    } else {
+        fuse = 1;
+    }
+    if (kernel == 3 && tile > 2) tile = 0;
+    if (kernel == 3 && fuse > 2 && tile == 2) tile = 1;
+    {
+        static const char *const names[5] = {"", "idg_naive_kernel", "idg_tiled_kernel", "idg_tma_kernel",
+                                             "idg_stream_kernel"};
+        snprintf(t_plan, sizeof(t_plan), "%s fuse=%d tile=%d", names[kernel], fuse, tile);
     }
 
     std::vector<idg::CubeParams> host_tab((size_t)batch);
@@ -147,8 +179,8 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     }
     for (int done = 0; done < max_n; done += fuse) {
         L.iter_done = done;
-        e = (kernel == 4)   ? idg::launch_stream(L, g_opt[IDG_OPT_CTAS], g_opt[IDG_OPT_TILE], st)
-            : (kernel == 3) ? idg::launch_tma(L, g_opt[IDG_OPT_ZCHUNK], g_opt[IDG_OPT_TILE], st)
+        e = (kernel == 4)   ? idg::launch_stream(L, g_opt[IDG_OPT_CTAS], tile, st)
+            : (kernel == 3) ? idg::launch_tma(L, g_opt[IDG_OPT_ZCHUNK], tile, st)
             : (kernel == 2) ? idg::launch_tiled(L, g_opt[IDG_OPT_ZCHUNK], st)
                             : idg::launch_naive(L, st);
         if (e != cudaSuccess) return (int)e;
@@ -276,7 +308,7 @@ int idg_set_option(int key, int value)
     if (key == IDG_OPT_KERNEL && (value < 0 || value > 4)) return IDG_ERR_OPTION;
     if (key == IDG_OPT_FUSE && (value < 0 || value > 4)) return IDG_ERR_OPTION;
     if (key == IDG_OPT_ZCHUNK && value < 0) return IDG_ERR_OPTION;
-    if (key == IDG_OPT_TILE && (value < 0 || value > 2)) return IDG_ERR_OPTION;
+    if (key == IDG_OPT_TILE && (value < 0 || value > 4)) return IDG_ERR_OPTION;
     if (key == IDG_OPT_CTAS && value < 0) return IDG_ERR_OPTION;
     g_opt[key] = value;
     return IDG_OK;
@@ -289,5 +321,7 @@ int idg_get_option(int key)
 }
 
 int idg_last_launch_count(void) { return t_launches; }
+
+const char *idg_last_plan(void) { return t_plan; }
 
 }  // extern "C"

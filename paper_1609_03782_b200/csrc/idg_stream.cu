@@ -338,34 +338,9 @@ __device__ __forceinline__ void run(const Launch &L, const StreamArgs &A, const 
             if (TL > 1) nw[0][r] = o;                       // level-1 plane q-1
             else if (st_on && (S.ok & (1u << r))) stg128(S.po + (long long)r * L.nx, o.x, o.y, o.z, o.w);
         }
-#pragma unroll
-        for (int t = 1; t < TL; ++t) {                      // level t -> t+1 from ring level t-1
-            const uint32_t e_self = sbase + Y::oEdge + (uint32_t)(t - 1) * Y::kEdgeLevel +
-                                    (uint32_t)(wy * 2 * kLanes + lane) * 16u;
-            const uint32_t wr = e_self + (par ^ 1u) * kParStride, rd = e_self + par * kParStride;
-            const F4 &e0 = nw[t - 1][0], &e1 = nw[t - 1][R - 1];
-            sts128(wr, e0.x, e0.y, e0.z, e0.w);
-            sts128(wr + kLanes * 16u, e1.x, e1.y, e1.z, e1.w);
-            const F4 up = ld4(rd - up_d * (kLanes * 16u));               // bottom row of strip wy-1
-            const F4 dn = ld4(rd + dn_d * (2u * kLanes * 16u));          // top row of strip wy+1
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const F4 &c = cc[t - 1][r];
-                float left = __shfl_up_sync(0xffffffffu, c.w, 1);
-                float right = __shfl_down_sync(0xffffffffu, c.x, 1);
-                left = first ? c.x : left;
-                right = last ? c.w : right;
-                const F4 &ym = (r == 0) ? up : cc[t - 1][r - 1];
-                const F4 &yp = (r == R - 1) ? dn : cc[t - 1][r + 1];
-                const F4 o = update4(c, left, right, ym, yp, zm[t - 1][r], nw[t - 1][r], kc);
-                if (t + 1 < TL) nw[t][r] = o;
-                else if (st_on && (S.ok & (1u << r))) stg128(S.po + (long long)r * L.nx, o.x, o.y, o.z, o.w);
-            }
-        }
-        // publish my edge rows, hand back the stage of plane q-2; the last warp to do so refills it
+        // all level-0 loads are done: hand back the stage of plane q-2; the last warp to do so refills it
         __syncwarp();
         if (lane == 0) {
-            mbar_arrive(nb_self + par * kNbPar);          // every step, so that phases track `it` in all runs
             const uint32_t cnt = sbase + Y::oCnt + s2 * 4u;
             if (atom_add_relaxed(cnt, 1u) == (uint32_t)(WARPS - 1)) {
                 sts32(cnt, 0u);
@@ -382,6 +357,35 @@ __device__ __forceinline__ void run(const Launch &L, const StreamArgs &A, const 
                 } else {
                     issue_ahead<TL, Y>(L, A, M, cur, NS - 2, s2, sbase);
                 }
+            }
+            if (TL == 1) mbar_arrive(nb_self + par * kNbPar);     // keeps the phases in step with `it`
+        }
+#pragma unroll
+        for (int t = 1; t < TL; ++t) {                      // level t -> t+1 from ring level t-1
+            const uint32_t e_self = sbase + Y::oEdge + (uint32_t)(t - 1) * Y::kEdgeLevel +
+                                    (uint32_t)(wy * 2 * kLanes + lane) * 16u;
+            const uint32_t wr = e_self + (par ^ 1u) * kParStride, rd = e_self + par * kParStride;
+            const F4 &e0 = nw[t - 1][0], &e1 = nw[t - 1][R - 1];
+            sts128(wr, e0.x, e0.y, e0.z, e0.w);
+            sts128(wr + kLanes * 16u, e1.x, e1.y, e1.z, e1.w);
+            const F4 up = ld4(rd - up_d * (kLanes * 16u));               // bottom row of strip wy-1
+            const F4 dn = ld4(rd + dn_d * (2u * kLanes * 16u));          // top row of strip wy+1
+            if (t == TL - 1) {      // last exchange of the step: my edge rows are published, the neighbours' read
+                __syncwarp();
+                if (lane == 0) mbar_arrive(nb_self + par * kNbPar);
+            }
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const F4 &c = cc[t - 1][r];
+                float left = __shfl_up_sync(0xffffffffu, c.w, 1);
+                float right = __shfl_down_sync(0xffffffffu, c.x, 1);
+                left = first ? c.x : left;
+                right = last ? c.w : right;
+                const F4 &ym = (r == 0) ? up : cc[t - 1][r - 1];
+                const F4 &yp = (r == R - 1) ? dn : cc[t - 1][r + 1];
+                const F4 o = update4(c, left, right, ym, yp, zm[t - 1][r], nw[t - 1][r], kc);
+                if (t + 1 < TL) nw[t][r] = o;
+                else if (st_on && (S.ok & (1u << r))) stg128(S.po + (long long)r * L.nx, o.x, o.y, o.z, o.w);
             }
         }
         P.it = it + 1;
@@ -561,14 +565,24 @@ bool stream_supported(int nx, int ny, int nz, const void *in, const void *out, c
 }
 
 // tile: 0 auto | 1 = 128x64 tile, 512 threads, one CTA per SM | 2 = 128x32 tile, 256 threads, two CTAs per SM
+//       | 3 = 128x40 tile, 320 threads, two CTAs per SM | 4 = 128x80 tile, 640 threads, one CTA per SM
 cudaError_t launch_stream(const Launch &L, int nctas, int tile, cudaStream_t st)
 {
-    const bool small = (tile == 2);
-    switch (L.fuse) {
-    case 1: return small ? launch_cfg<1, 4, 8, 5, 2>(L, nctas, st) : launch_cfg<1, 4, 16, 5, 1>(L, nctas, st);
-    case 2: return small ? launch_cfg<2, 4, 8, 5, 2>(L, nctas, st) : launch_cfg<2, 4, 16, 5, 1>(L, nctas, st);
-    case 3: return small ? launch_cfg<3, 4, 8, 5, 2>(L, nctas, st) : launch_cfg<3, 4, 16, 5, 1>(L, nctas, st);
-    case 4: return launch_cfg<4, 4, 12, 5, 1>(L, nctas, st);
+    switch (L.fuse * 10 + tile) {
+    case 10: case 11: return launch_cfg<1, 4, 16, 5, 1>(L, nctas, st);
+    case 12: return launch_cfg<1, 4, 8, 5, 2>(L, nctas, st);
+    case 13: return launch_cfg<1, 4, 10, 4, 2>(L, nctas, st);
+    case 14: return launch_cfg<1, 4, 20, 4, 1>(L, nctas, st);
+    case 20: case 21: return launch_cfg<2, 4, 16, 5, 1>(L, nctas, st);
+    case 22: return launch_cfg<2, 4, 8, 5, 2>(L, nctas, st);
+    case 23: return launch_cfg<2, 4, 10, 4, 2>(L, nctas, st);
+    case 24: return launch_cfg<2, 4, 20, 4, 1>(L, nctas, st);
+    case 30: case 31: return launch_cfg<3, 4, 16, 5, 1>(L, nctas, st);
+    case 32: return launch_cfg<3, 4, 8, 5, 2>(L, nctas, st);
+    case 33: return launch_cfg<3, 4, 12, 5, 1>(L, nctas, st);
+    case 34: return launch_cfg<3, 4, 14, 4, 1>(L, nctas, st);
+    case 40: case 41: return launch_cfg<4, 4, 12, 5, 1>(L, nctas, st);
+    case 42: return launch_cfg<4, 4, 8, 5, 1>(L, nctas, st);
     default: return cudaErrorInvalidValue;
     }
 }
