@@ -1,7 +1,8 @@
 """oracle/ -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
 
-Plain fp64 CPU oracle for the intensity-driven gradient filter (PAPER.md:165-189,
-section 3.3, Eq. 6-7), written from the paper and independent of the CUDA path:
+Plain fp64 CPU oracles for the intensity-driven gradient filter (PAPER.md:165-189,
+section 3.3, Eq. 6-7) and for the box and Gaussian reference filters (PAPER.md:121-159,
+sections 3.1-3.2, Eq. 1-3), written from the paper and independent of the CUDA path:
 it imports nothing from ``paper_1609_03782_b200`` and the package imports nothing
 from here.  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s
 ``cpu_baseline`` / ``--impl reference`` legs may use it.
@@ -47,6 +48,15 @@ def _load() -> ctypes.CDLL:
                                        ctypes.c_double, ctypes.c_double, ctypes.c_double, dp, dp]
         lib.idg_oracle_set_threads.restype = ctypes.c_int
         lib.idg_oracle_set_threads.argtypes = [ctypes.c_int]
+        ip = ctypes.POINTER(ctypes.c_int)
+        lib.box_oracle_f64.restype = ctypes.c_int
+        lib.box_oracle_f64.argtypes = [dp] + [ctypes.c_int] * 6 + [dp]
+        lib.gaussian_radii_oracle.restype = ctypes.c_int
+        lib.gaussian_radii_oracle.argtypes = [dp, dp, ip]
+        lib.gaussian_kernel_oracle.restype = ctypes.c_int
+        lib.gaussian_kernel_oracle.argtypes = [dp, dp, ip, dp]
+        lib.gaussian_oracle_f64.restype = ctypes.c_int
+        lib.gaussian_oracle_f64.argtypes = [dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp]
         _lib = lib
     return _lib
 
@@ -78,4 +88,63 @@ def idg_filter_oracle(cube: np.ndarray, n_iter: int, K: float = 1.5, tau: float 
                                 float(rms), out.ctypes.data_as(dp), scratch.ctypes.data_as(dp))
     if rc != 0:
         raise ValueError(f"idg_oracle_f64 rejected its arguments (rc={rc})")
+    return out
+
+
+def _cube64(cube: np.ndarray) -> np.ndarray:
+    a = np.ascontiguousarray(cube, dtype=np.float64)
+    if a.ndim != 3:
+        raise ValueError("cube must be 3-D [nz, ny, nx]")
+    return a
+
+
+def _d3(v) -> "ctypes.Array":
+    return (ctypes.c_double * 3)(*[float(t) for t in v])
+
+
+def box_filter_oracle(cube: np.ndarray, wx: int, wy: int, wz: int) -> np.ndarray:
+    """Box filter: mean over the wx x wy x wz neighbourhood (odd widths, x = RA) of
+    ``cube[z, y, x]``; out-of-cube neighbours are the nearest in-cube voxel (reading F1)."""
+    a = _cube64(cube)
+    nz, ny, nx = a.shape
+    out = np.empty_like(a)
+    dp = ctypes.POINTER(ctypes.c_double)
+    rc = _load().box_oracle_f64(a.ctypes.data_as(dp), nx, ny, nz, int(wx), int(wy), int(wz),
+                                out.ctypes.data_as(dp))
+    if rc != 0:
+        raise ValueError(f"box_oracle_f64 rejected its arguments (rc={rc})")
+    return out
+
+
+def gaussian_radii_oracle(fwhm, theta=(0.0, 0.0, 0.0)) -> tuple:
+    """Support radii (rx, ry, rz) of the sampled kernel (reading F3)."""
+    r = (ctypes.c_int * 3)()
+    if _load().gaussian_radii_oracle(_d3(fwhm), _d3(theta), r) != 0:
+        raise ValueError("invalid Gaussian parameters")
+    return int(r[0]), int(r[1]), int(r[2])
+
+
+def gaussian_kernel_oracle(fwhm, theta=(0.0, 0.0, 0.0)) -> np.ndarray:
+    """The normalised kernel of Eq. 1-3 as an array [2rz+1, 2ry+1, 2rx+1]; fwhm = (x, y, z) in voxels,
+    theta = (theta_x, theta_y, theta_z) in degrees."""
+    rx, ry, rz = gaussian_radii_oracle(fwhm, theta)
+    k = np.empty((2 * rz + 1, 2 * ry + 1, 2 * rx + 1), dtype=np.float64)
+    r = (ctypes.c_int * 3)(rx, ry, rz)
+    dp = ctypes.POINTER(ctypes.c_double)
+    if _load().gaussian_kernel_oracle(_d3(fwhm), _d3(theta), r, k.ctypes.data_as(dp)) != 0:
+        raise ValueError("invalid Gaussian parameters")
+    return k
+
+
+def gaussian_filter_oracle(cube: np.ndarray, fwhm, theta=(0.0, 0.0, 0.0)) -> np.ndarray:
+    """Gaussian filter (Eq. 1-3): direct 3-D convolution of ``cube[z, y, x]`` with the
+    kernel of :func:`gaussian_kernel_oracle`; replicated faces (reading F1)."""
+    a = _cube64(cube)
+    nz, ny, nx = a.shape
+    out = np.empty_like(a)
+    dp = ctypes.POINTER(ctypes.c_double)
+    rc = _load().gaussian_oracle_f64(a.ctypes.data_as(dp), nx, ny, nz, _d3(fwhm), _d3(theta),
+                                     out.ctypes.data_as(dp))
+    if rc != 0:
+        raise ValueError(f"gaussian_oracle_f64 rejected its arguments (rc={rc})")
     return out
