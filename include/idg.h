@@ -12,7 +12,8 @@
  * update is Jacobi (two buffers); an out-of-cube neighbour
  * equals the centre voxel (zero-flux boundary, reading R1); rms is a
  * caller-supplied constant.  All arithmetic runs in hand-written sm_100a CUDA
- * kernels; there is no CPU fallback.
+ * kernels; there is no CPU fallback.  The library also holds the paper's two reference filters
+ * (box, Gaussian; sections 3.1-3.2), declared after the IDG entry points.
  *
  * Conventions for every entry point
  *   layout    dense, idx = x + nx*(y + ny*z); x = RA (fastest), y = Dec,
@@ -128,6 +129,39 @@ int idg_filter_batched(const float *cubes, int nx, int ny, int nz, int batch,
 int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
                     const idg_params *params, float *out_host,
                     void *dev_buffers, size_t dev_buffers_bytes, void *stream);
+
+/*
+ * Box filter (section 3.1): every voxel becomes the mean of its wx x wy x wz
+ * neighbourhood, itself included (the paper's N_x, N_y, N_z).  Out-of-cube
+ * neighbours are the nearest in-cube voxel (reading F1).  One fused separable pass.
+ *   cube [device] nx*ny*nz fp32;  out [device] nx*ny*nz fp32, must not overlap cube
+ *   wx, wy, wz   odd, 1 .. 33 (wx along x = RA); anything else returns IDG_ERR_PARAM
+ */
+int idg_box_filter(const float *cube, int nx, int ny, int nz, int wx, int wy, int wz, float *out, void *stream);
+
+/*
+ * Gaussian filter (section 3.2): 3-D convolution with
+ *   G = A exp(-(x^2/2sx^2 + y^2/2sy^2 + z^2/2sz^2))  (Eq. 1),  FWHM_j = 2 sqrt(2 ln 2) s_j  (Eq. 2),
+ *   K = Rz(theta_z) Ry(theta_y) Rx(theta_x) G        (Eq. 3).
+ * Readings (F1-F5): replicated faces; the sampled kernel is normalised to unit sum;
+ * support |p_j| <= floor(3 s_j + 1/2), for a rotated kernel the cube of the largest such radius;
+ * (R G)(p) = G(R^-1 p) with right-handed matrices, angles in degrees; FWHM_j = 0 switches axis j off
+ * (not allowed together with a rotation).  All angles zero: one fused separable pass (radius <= 16
+ * per axis, FWHM <= 12.9); otherwise a dense (2r+1)^3 convolution (r <= 10, FWHM <= 8.2).  Parameters
+ * outside these limits, negative or non-finite return IDG_ERR_PARAM.
+ *   cube [device] nx*ny*nz fp32;  out [device] nx*ny*nz fp32, must not overlap cube
+ *   fwhm_* in voxels, theta_* in degrees.  The rotated path takes (2r+1)^3 floats from the
+ *   stream-ordered allocator for the kernel weights and returns them before the call returns.
+ */
+int idg_gaussian_filter(const float *cube, int nx, int ny, int nz, float fwhm_x, float fwhm_y, float fwhm_z,
+                        float theta_x, float theta_y, float theta_z, float *out, void *stream);
+
+/*
+ * Host-only: support radii (rx, ry, rz) idg_gaussian_filter would use, or IDG_ERR_PARAM.
+ *   radii [host] 3 ints
+ */
+int idg_gaussian_radii(float fwhm_x, float fwhm_y, float fwhm_z, float theta_x, float theta_y, float theta_z,
+                       int radii[3]);
 
 /*
  * Process-wide tuning knobs (tests and benchmarks; defaults give the fastest plan).

@@ -23,7 +23,8 @@ KERNEL_AUTO, KERNEL_NAIVE, KERNEL_TILED, KERNEL_TMA, KERNEL_STREAM = 0, 1, 2, 3,
 # every symbol include/idg.h declares (tests check the library exports them all)
 SYMBOLS = ("idg_version", "idg_status_string", "idg_params_check", "idg_workspace_bytes",
            "idg_filter", "idg_filter_ws", "idg_filter_batched", "idg_filter_host",
-           "idg_set_option", "idg_get_option", "idg_last_launch_count", "idg_last_plan")
+           "idg_set_option", "idg_get_option", "idg_last_launch_count", "idg_last_plan",
+           "idg_box_filter", "idg_gaussian_filter", "idg_gaussian_radii")
 
 
 class IdgParams(ctypes.Structure):
@@ -90,6 +91,13 @@ def lib() -> ctypes.CDLL:
         L.idg_get_option.argtypes = [i]
         L.idg_last_launch_count.restype = i
         L.idg_last_plan.restype = ctypes.c_char_p
+        f = ctypes.c_float
+        L.idg_box_filter.restype = i
+        L.idg_box_filter.argtypes = [fp, i, i, i, i, i, i, fp, vp]
+        L.idg_gaussian_filter.restype = i
+        L.idg_gaussian_filter.argtypes = [fp, i, i, i, f, f, f, f, f, f, fp, vp]
+        L.idg_gaussian_radii.restype = i
+        L.idg_gaussian_radii.argtypes = [f, f, f, f, f, f, ctypes.POINTER(ctypes.c_int)]
         _lib = L
     return _lib
 
@@ -214,6 +222,41 @@ def idg_filter_host(cube_host: torch.Tensor, n_iter: int, params: Params = Param
                                out_host.data_ptr(), dptr, dbytes, _stream(stream))
     _check(rc)
     return out_host
+
+
+def idg_box_filter(cube: torch.Tensor, wx: int, wy: int, wz: int, out: Optional[torch.Tensor] = None,
+                   stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """idg_box_filter on a [nz, ny, nx] CUDA tensor (widths along x, y, z).  Asynchronous on `stream`."""
+    if cube.dim() != 3:
+        raise ValueError("cube must be [nz, ny, nx]")
+    nz, ny, nx = cube.shape
+    if out is None:
+        out = torch.empty_like(cube)
+    _check(lib().idg_box_filter(_dev(cube, "cube"), nx, ny, nz, int(wx), int(wy), int(wz), _dev(out, "out"),
+                                _stream(stream)))
+    return out
+
+
+def idg_gaussian_filter(cube: torch.Tensor, fwhm: Sequence[float], theta: Sequence[float] = (0.0, 0.0, 0.0),
+                        out: Optional[torch.Tensor] = None,
+                        stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """idg_gaussian_filter on a [nz, ny, nx] CUDA tensor; fwhm = (x, y, z) voxels, theta = (x, y, z) degrees."""
+    if cube.dim() != 3:
+        raise ValueError("cube must be [nz, ny, nx]")
+    nz, ny, nx = cube.shape
+    if out is None:
+        out = torch.empty_like(cube)
+    _check(lib().idg_gaussian_filter(_dev(cube, "cube"), nx, ny, nz, float(fwhm[0]), float(fwhm[1]),
+                                     float(fwhm[2]), float(theta[0]), float(theta[1]), float(theta[2]),
+                                     _dev(out, "out"), _stream(stream)))
+    return out
+
+
+def idg_gaussian_radii(fwhm: Sequence[float], theta: Sequence[float] = (0.0, 0.0, 0.0)) -> tuple:
+    r = (ctypes.c_int * 3)()
+    _check(lib().idg_gaussian_radii(float(fwhm[0]), float(fwhm[1]), float(fwhm[2]), float(theta[0]),
+                                    float(theta[1]), float(theta[2]), r))
+    return int(r[0]), int(r[1]), int(r[2])
 
 
 def host_buffers_bytes(nx: int, ny: int, nz: int) -> int:

@@ -302,6 +302,135 @@ int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
     return e3 == cudaSuccess ? IDG_OK : (int)e3;
 }
 
+// ---- reference filters (PAPER.md sections 3.1-3.2) -------------------------------------------
+
+static int ref_args(const float *cube, int nx, int ny, int nz, const float *out, size_t *N)
+{
+    if (!cube || !out) return IDG_ERR_NULL;
+    if (!voxel_count(nx, ny, nz, 1, N)) return IDG_ERR_DIMS;
+    if (ranges_overlap(cube, *N * sizeof(float), out, *N * sizeof(float))) return IDG_ERR_OVERLAP;
+    return IDG_OK;
+}
+
+int idg_box_filter(const float *cube, int nx, int ny, int nz, int wx, int wy, int wz, float *out, void *stream)
+{
+    t_launches = 0;
+    size_t N;
+    const int rc = ref_args(cube, nx, ny, nz, out, &N);
+    if (rc != IDG_OK) return rc;
+    const int w[3] = {wx, wy, wz};
+    float wt[3][2 * idg::kSepMaxRadius + 1];
+    for (int a = 0; a < 3; ++a) {
+        if (w[a] < 1 || !(w[a] & 1) || w[a] > 2 * idg::kSepMaxRadius + 1) return IDG_ERR_PARAM;
+        for (int i = 0; i < w[a]; ++i) wt[a][i] = (float)(1.0 / (double)w[a]);     // PAPER.md:123, the mean
+    }
+    const cudaError_t e = idg::launch_sep3d(cube, out, nx, ny, nz, wx / 2, wy / 2, wz / 2, wt[0], wt[1], wt[2],
+                                            (cudaStream_t)stream);
+    if (e != cudaSuccess) return (int)e;
+    t_launches = 1;
+    snprintf(t_plan, sizeof(t_plan), "idg_sep3d_kernel box %dx%dx%d", wx, wy, wz);
+    return IDG_OK;
+}
+
+// Eq. 2 and reading F3: sigma and support radius of one axis.
+static double sigma_of(double fwhm) { return fwhm / (2.0 * sqrt(2.0 * log(2.0))); }
+static int radius_of(double sigma) { return (int)floor(3.0 * sigma + 0.5); }
+
+int idg_gaussian_radii(float fwhm_x, float fwhm_y, float fwhm_z, float theta_x, float theta_y, float theta_z,
+                       int radii[3])
+{
+    if (!radii) return IDG_ERR_NULL;
+    const double f[3] = {fwhm_x, fwhm_y, fwhm_z}, th[3] = {theta_x, theta_y, theta_z};
+    for (int a = 0; a < 3; ++a)
+        if (!(f[a] >= 0.0) || !isfinite(f[a]) || !isfinite(th[a])) return IDG_ERR_PARAM;
+    const bool rotated = th[0] != 0.0 || th[1] != 0.0 || th[2] != 0.0;
+    if (rotated) {
+        double smax = 0.0;
+        for (int a = 0; a < 3; ++a) {
+            if (!(f[a] > 0.0)) return IDG_ERR_PARAM;                         // reading F5
+            smax = fmax(smax, sigma_of(f[a]));
+        }
+        radii[0] = radii[1] = radii[2] = radius_of(smax);
+        if (radii[0] > idg::kConvMaxRadius) return IDG_ERR_PARAM;
+    } else {
+        for (int a = 0; a < 3; ++a) {
+            radii[a] = radius_of(sigma_of(f[a]));
+            if (radii[a] > idg::kSepMaxRadius) return IDG_ERR_PARAM;
+        }
+    }
+    return IDG_OK;
+}
+
+int idg_gaussian_filter(const float *cube, int nx, int ny, int nz, float fwhm_x, float fwhm_y, float fwhm_z,
+                        float theta_x, float theta_y, float theta_z, float *out, void *stream)
+{
+    t_launches = 0;
+    size_t N;
+    int rc = ref_args(cube, nx, ny, nz, out, &N);
+    if (rc != IDG_OK) return rc;
+    int r[3];
+    rc = idg_gaussian_radii(fwhm_x, fwhm_y, fwhm_z, theta_x, theta_y, theta_z, r);
+    if (rc != IDG_OK) return rc;
+    const double f[3] = {fwhm_x, fwhm_y, fwhm_z}, th[3] = {theta_x, theta_y, theta_z};
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool rotated = th[0] != 0.0 || th[1] != 0.0 || th[2] != 0.0;
+    if (!rotated) {
+        // Eq. 1 factorises along the axes: three 1-D kernels, each normalised to unit sum (reading F2)
+        float wt[3][2 * idg::kSepMaxRadius + 1];
+        for (int a = 0; a < 3; ++a) {
+            const double s = sigma_of(f[a]);
+            double g[2 * idg::kSepMaxRadius + 1], sum = 0.0;
+            for (int i = -r[a]; i <= r[a]; ++i) {
+                g[i + r[a]] = s > 0.0 ? exp(-(double)(i * i) / (2.0 * s * s)) : 1.0;
+                sum += g[i + r[a]];
+            }
+            for (int i = 0; i <= 2 * r[a]; ++i) wt[a][i] = (float)(g[i] / sum);
+        }
+        const cudaError_t e = idg::launch_sep3d(cube, out, nx, ny, nz, r[0], r[1], r[2], wt[0], wt[1], wt[2], st);
+        if (e != cudaSuccess) return (int)e;
+        t_launches = 1;
+        snprintf(t_plan, sizeof(t_plan), "idg_sep3d_kernel gauss r=%d,%d,%d", r[0], r[1], r[2]);
+        return IDG_OK;
+    }
+    // Eq. 3: K(p) = G(R^-1 p), R = Rz Ry Rx (right-handed, degrees), sampled on the cube |p_j| <= r
+    const double d2r = acos(-1.0) / 180.0;
+    const double cx = cos(th[0] * d2r), sx = sin(th[0] * d2r), cy = cos(th[1] * d2r), sy = sin(th[1] * d2r),
+                 cz = cos(th[2] * d2r), sz = sin(th[2] * d2r);
+    const double R[3][3] = {{cz * cy, cz * sy * sx - sz * cx, cz * sy * cx + sz * sx},
+                            {sz * cy, sz * sy * sx + cz * cx, sz * sy * cx - cz * sx},
+                            {-sy, cy * sx, cy * cx}};
+    double i2[3];
+    for (int a = 0; a < 3; ++a) i2[a] = 1.0 / (2.0 * sigma_of(f[a]) * sigma_of(f[a]));
+    const int rr = r[0], W = 2 * rr + 1;
+    std::vector<double> g((size_t)W * W * W);
+    double sum = 0.0;
+    size_t m = 0;
+    for (int k = -rr; k <= rr; ++k)
+        for (int j = -rr; j <= rr; ++j)
+            for (int i = -rr; i <= rr; ++i) {
+                double q2 = 0.0;
+                for (int a = 0; a < 3; ++a) {
+                    const double q = R[0][a] * i + R[1][a] * j + R[2][a] * k;      // (R^T p)_a
+                    q2 += q * q * i2[a];
+                }
+                g[m] = exp(-q2);
+                sum += g[m++];
+            }
+    std::vector<float> gf(g.size());
+    for (size_t t = 0; t < g.size(); ++t) gf[t] = (float)(g[t] / sum);
+    float *d_k = nullptr;
+    cudaError_t e = cudaMallocAsync((void **)&d_k, gf.size() * sizeof(float), st);
+    if (e != cudaSuccess) return (int)e;
+    e = cudaMemcpyAsync(d_k, gf.data(), gf.size() * sizeof(float), cudaMemcpyHostToDevice, st);   // pageable: staged before return
+    if (e == cudaSuccess) e = idg::launch_conv3d(cube, out, nx, ny, nz, rr, d_k, st);
+    const cudaError_t e2 = cudaFreeAsync(d_k, st);
+    if (e != cudaSuccess) return (int)e;
+    if (e2 != cudaSuccess) return (int)e2;
+    t_launches = 1;
+    snprintf(t_plan, sizeof(t_plan), "idg_conv3d_kernel<r=%d>", rr);
+    return IDG_OK;
+}
+
 int idg_set_option(int key, int value)
 {
     if (key < 0 || key >= IDG_OPT_COUNT_) return IDG_ERR_OPTION;

@@ -86,4 +86,15 @@ bool tma_supported(int nx, int ny, int nz, const void *in, const void *out, cons
 cudaError_t launch_stream(const Launch &L, int nctas, int tile, cudaStream_t st);
 bool stream_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
 
+
+// Reference filters (PAPER.md sections 3.1-3.2): separable single-pass filter (box, axis-aligned
+// Gaussian) and dense 3-D convolution (rotated Gaussian, Eq. 3).
+constexpr int kSepMaxRadius = 16;      // per-axis radius limit of the separable kernel
+constexpr int kConvMaxRadius = 10;     // radius limit of the dense kernel (cube support (2r+1)^3)
+cudaError_t launch_sep3d(const float *in, float *out, int nx, int ny, int nz, int rx, int ry, int rz,
+                         const float *wx, const float *wy, const float *wz, cudaStream_t st);
+// kern [device]: (2r+1)^3 weights, x fastest
+cudaError_t launch_conv3d(const float *in, float *out, int nx, int ny, int nz, int r, const float *kern,
+                          cudaStream_t st);
+
 }  // namespace idg

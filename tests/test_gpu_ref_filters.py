@@ -1,0 +1,115 @@
+"""GPU parity of the reference filters (box, Gaussian; PAPER.md sections 3.1-3.2, Eq. 1-3): the CUDA
+path through the C ABI against the direct-sum fp64 oracle, element by element.
+
+The GPU path is separable and fused (idg_sep3d_kernel) or a dense register-blocked convolution
+(idg_conv3d_kernel); the oracle is the plain 3-D sum, so agreement checks the algorithm as well as
+the arithmetic.  Bar: max |gpu - oracle| <= 1e-4 * noise rms (the north_star tolerance; the fp32
+sums of at most 9261 terms stay two orders of magnitude below it).
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1609_03782_b200 import binding
+    binding.lib()
+    return binding
+
+
+def noisy(shape, seed):
+    rng = np.random.default_rng(seed)
+    return (rng.normal(0, 1, shape) + 8.0 * (rng.random(shape) < 0.03)).astype(np.float32)
+
+
+def err(out, ref):
+    return float(np.abs(out.cpu().numpy().astype(np.float64) - ref).max())
+
+
+SHAPES = [(1, 1, 1), (5, 7, 9), (3, 20, 70), (21, 67, 100), (40, 50, 130), (70, 17, 64), (9, 33, 260)]
+IDS = lambda s: "x".join(map(str, s[::-1])) if isinstance(s, tuple) and len(s) == 3 else None
+
+
+@pytest.mark.parametrize("w", [(1, 1, 1), (3, 3, 3), (3, 5, 5), (9, 9, 9), (33, 1, 7), (5, 33, 1)], ids=str)
+@pytest.mark.parametrize("shape", SHAPES, ids=IDS)
+def test_box(B, oracle, shape, w):
+    """Paper widths N_j = 1..9, isotropic and anisotropic, and the
+    library limit 33; cubes smaller than the kernel, ragged tile tails, several z chunks."""
+    a = noisy(shape, 11)
+    out = B.idg_box_filter(torch.from_numpy(a).cuda(), *w)
+    torch.cuda.synchronize()
+    assert err(out, oracle.box_filter_oracle(a, *w)) <= TOL
+
+
+@pytest.mark.parametrize("fwhm", [(3, 3, 3), (2, 3, 3), (7, 3, 3), (1, 5, 3), (0, 3, 0), (12.9, 1, 1)], ids=str)
+@pytest.mark.parametrize("shape", SHAPES, ids=IDS)
+def test_gaussian_axis_aligned(B, oracle, shape, fwhm):
+    """theta = 0: separable path; paper FWHM 1..7 and the library limit."""
+    a = noisy(shape, 12)
+    out = B.idg_gaussian_filter(torch.from_numpy(a).cuda(), fwhm)
+    torch.cuda.synchronize()
+    assert err(out, oracle.gaussian_filter_oracle(a, fwhm)) <= TOL
+    assert B.idg_gaussian_radii(fwhm) == oracle.gaussian_radii_oracle(fwhm)
+
+
+@pytest.mark.parametrize("case", [((3, 3, 3), (10, 20, 30)), ((2, 3, 3), (0, 0, 45)), ((7, 3, 3), (90, 0, 90)),
+                                  ((7, 3, 3), (25, -40, 110)), ((1, 1, 1), (5, 5, 5)), ((8.2, 2, 4), (0, 33, 0))],
+                         ids=str)
+@pytest.mark.parametrize("shape", [(5, 7, 9), (21, 30, 70), (17, 9, 33)], ids=IDS)
+def test_gaussian_rotated(B, oracle, shape, case):
+    """Eq. 3: dense kernel, r = 1 .. 10; Table 2 of the paper rotates FWHM (7, 3, 3)."""
+    fwhm, theta = case
+    a = noisy(shape, 13)
+    out = B.idg_gaussian_filter(torch.from_numpy(a).cuda(), fwhm, theta)
+    torch.cuda.synchronize()
+    assert err(out, oracle.gaussian_filter_oracle(a, fwhm, theta)) <= TOL
+    assert B.idg_gaussian_radii(fwhm, theta) == oracle.gaussian_radii_oracle(fwhm, theta)
+
+
+def test_config0_cube_with_the_papers_timing_parameters(B, oracle):
+    """The four reference-filter settings the paper times on the config-0 cube."""
+    from paper_1609_03782_b200 import synth
+    c = synth.modelb_like(seed=1000, snr=32.0)
+    t = torch.from_numpy(c.data).cuda()
+    assert err(B.idg_box_filter(t, 3, 3, 3), oracle.box_filter_oracle(c.data, 3, 3, 3)) <= TOL * c.rms
+    assert err(B.idg_box_filter(t, 3, 5, 5), oracle.box_filter_oracle(c.data, 3, 5, 5)) <= TOL * c.rms
+    assert err(B.idg_gaussian_filter(t, (3, 3, 3)), oracle.gaussian_filter_oracle(c.data, (3, 3, 3))) <= TOL * c.rms
+    assert err(B.idg_gaussian_filter(t, (2, 3, 3)), oracle.gaussian_filter_oracle(c.data, (2, 3, 3))) <= TOL * c.rms
+    assert err(B.idg_gaussian_filter(t, (2, 3, 3), (30, 0, 60)),
+               oracle.gaussian_filter_oracle(c.data, (2, 3, 3), (30, 0, 60))) <= TOL * c.rms
+
+
+def test_invariants_on_gpu(B):
+    """Constant cube is a fixed point (unit-sum weights, to fp32 rounding); width 1 / FWHM 0 copy."""
+    t = torch.full((20, 40, 72), 2.5, device="cuda")
+    for out in (B.idg_box_filter(t, 5, 5, 5), B.idg_gaussian_filter(t, (3, 3, 3)),
+                B.idg_gaussian_filter(t, (3, 2, 4), (10, 20, 30))):
+        assert float((out - t).abs().max()) <= 2.5 * 2e-6
+    a = torch.from_numpy(noisy((9, 20, 33), 5)).cuda()
+    assert torch.equal(B.idg_box_filter(a, 1, 1, 1), a)
+    assert torch.equal(B.idg_gaussian_filter(a, (0, 0, 0)), a)
+
+
+def test_argument_errors(B):
+    a = torch.zeros((4, 5, 8), device="cuda")
+    for w in ((2, 3, 3), (3, 0, 3), (3, 3, 35)):
+        with pytest.raises(B.IdgError) as e:
+            B.idg_box_filter(a, *w)
+        assert e.value.status == -4
+    with pytest.raises(B.IdgError) as e:
+        B.idg_box_filter(a, 3, 3, 3, out=a)
+    assert e.value.status == -6
+    for fwhm, theta in (((-1, 3, 3), (0, 0, 0)), ((14, 3, 3), (0, 0, 0)), ((9, 3, 3), (0, 0, 10)),
+                        ((0, 3, 3), (0, 0, 10)), ((float("nan"), 3, 3), (0, 0, 0))):
+        with pytest.raises(B.IdgError) as e:
+            B.idg_gaussian_filter(a, fwhm, theta)
+        assert e.value.status == -4
+    with pytest.raises(TypeError):
+        B.idg_box_filter(a.cpu(), 3, 3, 3)
