@@ -177,6 +177,22 @@ def run_reference(args) -> None:
     }))
 
 
+def max_over_ranks(ms: float, world: int, device) -> float:
+    """Slowest rank's time (the contract's max over ranks); a collective every rank must enter."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(voxel_iters_per_rank: float, world: int, ms_step_max: float) -> float:
+    """Whole-job throughput: the units all ranks processed / the slowest rank's time, in G/s."""
+    return world * voxel_iters_per_rank / (ms_step_max * 1e-3) / 1e9
+
+
 def run_ours(args) -> None:
     import torch
     import torch.distributed as dist
@@ -232,11 +248,8 @@ def run_ours(args) -> None:
     barrier()
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop() if rank == 0 else {}
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step = float(t.item()) / args.steps
-    value = world * N * n / (ms_step * 1e-3) / 1e9
+    ms_step = max_over_ranks(ms, world, "cuda") / args.steps
+    value = aggregate_value(N * n, world, ms_step)
 
     # end to end through the C-ABI host entry point: pinned host buffers, copies inside the timed region
     e2e_value = None
@@ -254,10 +267,7 @@ def run_ours(args) -> None:
         e1.record(stream)
         barrier()
         e_ms = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3)
-        t = torch.tensor([e_ms], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_value = world * N * n / (float(t.item()) / e_steps * 1e-3) / 1e9
+        e2e_value = aggregate_value(N * n, world, max_over_ranks(e_ms, world, "cuda") / e_steps)
 
     if rank != 0:
         if world > 1:
