@@ -73,6 +73,22 @@ __device__ __forceinline__ void ypass(const float *B, const SepArgs &S, int yg, 
     }
 }
 
+// z pass: combine the 2R+1 ring planes, starting at ring slot `sl` (the plane zo - R), for my 4 rows.
+template <int R>
+__device__ __forceinline__ void zpass(const float *ring_col, int sl, const SepArgs &S, float (&acc)[4])
+{
+    constexpr int W = 2 * R + 1;
+#pragma unroll
+    for (int o = 0; o < 4; ++o) acc[o] = 0.f;
+#pragma unroll
+    for (int k = 0; k < W; ++k) {
+        const float wk = S.wz[k];
+#pragma unroll
+        for (int o = 0; o < 4; ++o) acc[o] = fmaf(wk, ring_col[(sl * TY + o) * TX], acc[o]);
+        sl = (sl + 1 == W) ? 0 : sl + 1;
+    }
+}
+
 #define IDG_SEP_SWITCH(r, CALL)                                                                      \
     switch (r) {                                                                                     \
     case 0: { constexpr int R_ = 0; CALL; } break;   case 1: { constexpr int R_ = 1; CALL; } break;   \
@@ -89,13 +105,13 @@ __device__ __forceinline__ void ypass(const float *B, const SepArgs &S, int yg, 
 constexpr int kRowIters = (TY + 2 * kSepMaxRadius + NT / 32 - 1) / (NT / 32);   // halo rows per warp: <= 6
 constexpr int kColIters = (TX + 2 * kSepMaxRadius + 31) / 32;                    // halo columns per lane: <= 3
 
-__global__ void __launch_bounds__(NT) idg_sep3d_kernel(const __grid_constant__ SepArgs S)
+__global__ void __launch_bounds__(NT, 3) idg_sep3d_kernel(const __grid_constant__ SepArgs S)
 {
     extern __shared__ __align__(16) float smem[];
     const int stride = TX + 2 * S.hx;
     const int rows = TY + 2 * S.ry;
     float *A = smem;                                  // rows x stride   input tile with halo
-    float *B = A + rows * stride;                     // rows x TX       after the x pass
+    float *B = A + ((rows + 7) & ~7) * stride;        // rows x TX       after the x pass (A padded to 8 rows)
     float *ring = B + rows * TX;                      // (2rz+1) x TY x TX   xy-filtered planes
     const int W = 2 * S.rz + 1;
 
@@ -114,34 +130,38 @@ __global__ void __launch_bounds__(NT) idg_sep3d_kernel(const __grid_constant__ S
 #pragma unroll
     for (int c = 0; c < kColIters; ++c) gxo[c] = min(max(x0 - S.rx + lane + 32 * c, 0), S.nx - 1);
 
+    // rows are padded to a multiple of 8 in A (the extra rows reload clamped rows and are never read)
+    const int n_it = (rows + NT / 32 - 1) / (NT / 32);
+    const bool c2 = lane + 64 < cols;                 // columns lane, lane+32 always exist (cols >= 64)
     float pre[kRowIters * kColIters];
     auto fetch = [&](int q) {                         // plane clamp(q) -> registers
         const float *src = S.in + (size_t)min(max(q, 0), S.nz - 1) * plane;
 #pragma unroll
         for (int i = 0; i < kRowIters; ++i) {
-            const int row = warp + (NT / 32) * i;
-            if (row < rows) {
-                const float *rp = src + (size_t)min(max(y0 - S.ry + row, 0), S.ny - 1) * S.nx;
-#pragma unroll
-                for (int c = 0; c < kColIters; ++c)
-                    if (lane + 32 * c < cols) pre[i * kColIters + c] = __ldg(rp + gxo[c]);
+            if (i < n_it) {
+                const float *rp = src + (size_t)min(max(y0 - S.ry + warp + (NT / 32) * i, 0), S.ny - 1) * S.nx;
+                pre[i * kColIters + 0] = __ldg(rp + gxo[0]);
+                pre[i * kColIters + 1] = __ldg(rp + gxo[1]);
+                if (c2) pre[i * kColIters + 2] = __ldg(rp + gxo[2]);
             }
         }
     };
+    float *a_thr = A + warp * stride + S.hx - S.rx + lane;
     auto stash = [&]() {                              // registers -> A
 #pragma unroll
         for (int i = 0; i < kRowIters; ++i) {
-            const int row = warp + (NT / 32) * i;
-            if (row < rows) {
-#pragma unroll
-                for (int c = 0; c < kColIters; ++c)
-                    if (lane + 32 * c < cols) A[row * stride + S.hx - S.rx + lane + 32 * c] = pre[i * kColIters + c];
+            if (i < n_it) {
+                float *ap = a_thr + (NT / 32) * i * stride;
+                ap[0] = pre[i * kColIters + 0];
+                ap[32] = pre[i * kColIters + 1];
+                if (c2) ap[64] = pre[i * kColIters + 2];
             }
         }
     };
 
     const int q_first = z0 - S.rz, q_last = z1 - 1 + S.rz;
     fetch(q_first);
+    int slot = 0;
     for (int q = q_first; q <= q_last; ++q) {
         stash();
         __syncthreads();                              // A complete; everybody is done with B of the previous plane
@@ -150,19 +170,16 @@ __global__ void __launch_bounds__(NT) idg_sep3d_kernel(const __grid_constant__ S
         __syncthreads();                              // B complete; A may be overwritten
         float p[4];
         IDG_SEP_SWITCH(S.ry, ypass<R_>(B, S, yg, xl, p));
-        // my four ring entries of slot q mod W (private to this thread)
-        const int slot = ((q % W) + W) % W;
+        // my four ring entries of the slot of plane q (private to this thread)
+        float *ring_col = ring + (4 * yg) * TX + xl;
 #pragma unroll
-        for (int o = 0; o < 4; ++o) ring[(slot * TY + 4 * yg + o) * TX + xl] = p[o];
+        for (int o = 0; o < 4; ++o) ring_col[(slot * TY + o) * TX] = p[o];
         const int zo = q - S.rz;                      // output plane whose window [zo-rz, zo+rz] is now complete
+        const int slot0 = (slot + 1 == W) ? 0 : slot + 1;     // slot of plane q - 2rz = zo - rz
+        slot = slot0;                                 // = slot of plane q + 1
         if (zo >= z0) {
-            float acc[4] = {0.f, 0.f, 0.f, 0.f};
-            for (int k = 0; k < W; ++k) {
-                const int sl = (((zo - S.rz + k) % W) + W) % W;
-                const float wk = S.wz[k];
-#pragma unroll
-                for (int o = 0; o < 4; ++o) acc[o] = fmaf(wk, ring[(sl * TY + 4 * yg + o) * TX + xl], acc[o]);
-            }
+            float acc[4];
+            IDG_SEP_SWITCH(S.rz, zpass<R_>(ring_col, slot0, S, acc));
             if (col_ok) {
                 float *dst = S.out + (size_t)zo * plane + (size_t)(y0 + 4 * yg) * S.nx + x0 + xl;
 #pragma unroll
@@ -203,7 +220,7 @@ cudaError_t launch_sep3d(const float *in, float *out, int nx, int ny, int nz, in
     chunks = (nz + S.zchunk - 1) / S.zchunk;
     if (tiles_y > 65535 || chunks > 65535) return cudaErrorInvalidValue;
     const int rows = TY + 2 * ry, stride = TX + 2 * S.hx;
-    const size_t smem = sizeof(float) * ((size_t)rows * stride + (size_t)rows * TX + (size_t)(2 * rz + 1) * TY * TX);
+    const size_t smem = sizeof(float) * ((size_t)((rows + 7) & ~7) * stride + (size_t)rows * TX + (size_t)(2 * rz + 1) * TY * TX);
     static size_t attr = 0;
     if (smem > attr) {
         cudaError_t e = cudaFuncSetAttribute(idg_sep3d_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -54,7 +54,6 @@ __device__ __forceinline__ F4 ld4(uint32_t a)
     const float4 v = lds128(a);
     return F4{v.x, v.y, v.z, v.w};
 }
-__device__ __forceinline__ F4 reversed(const F4 &a) { return F4{a.w, a.z, a.y, a.x}; }
 
 // Four voxel updates of one float4 column with packed fp32x2 arithmetic.  Each component rounds
 // exactly like the scalar update() of idg_kernels.cuh (same operations in the same order).
@@ -571,16 +570,16 @@ cudaError_t launch_stream(const Launch &L, int nctas, int tile, cudaStream_t st)
     switch (L.fuse * 10 + tile) {
     case 10: case 11: return launch_cfg<1, 4, 16, 5, 1>(L, nctas, st);
     case 12: return launch_cfg<1, 4, 8, 5, 2>(L, nctas, st);
-    case 13: return launch_cfg<1, 4, 10, 4, 2>(L, nctas, st);
-    case 14: return launch_cfg<1, 4, 20, 4, 1>(L, nctas, st);
+    case 13: return launch_cfg<1, 4, 20, 5, 1>(L, nctas, st);
+    case 14: return launch_cfg<1, 4, 10, 5, 2>(L, nctas, st);
     case 20: case 21: return launch_cfg<2, 4, 16, 5, 1>(L, nctas, st);
     case 22: return launch_cfg<2, 4, 8, 5, 2>(L, nctas, st);
-    case 23: return launch_cfg<2, 4, 10, 4, 2>(L, nctas, st);
-    case 24: return launch_cfg<2, 4, 20, 4, 1>(L, nctas, st);
+    case 23: return launch_cfg<2, 3, 20, 5, 1>(L, nctas, st);
+    case 24: return launch_cfg<2, 3, 16, 5, 1>(L, nctas, st);
     case 30: case 31: return launch_cfg<3, 4, 16, 5, 1>(L, nctas, st);
     case 32: return launch_cfg<3, 4, 8, 5, 2>(L, nctas, st);
     case 33: return launch_cfg<3, 4, 12, 5, 1>(L, nctas, st);
-    case 34: return launch_cfg<3, 4, 14, 4, 1>(L, nctas, st);
+    case 34: return launch_cfg<3, 3, 16, 5, 1>(L, nctas, st);
     case 40: case 41: return launch_cfg<4, 4, 12, 5, 1>(L, nctas, st);
     case 42: return launch_cfg<4, 4, 8, 5, 1>(L, nctas, st);
     default: return cudaErrorInvalidValue;
