@@ -36,7 +36,13 @@ WORKLOADS = {
     "cfg3_1024x1024x512_n20": ((512, 1024, 1024), 20, "large"),
     "cfg2_512x512x256_n20": ((256, 512, 512), 20, "survey"),
     "cfg0_100x100x67_n10": ((67, 100, 100), 10, "modelb"),
+    "cfg4_256x128x128x64_n10": ((64, 128, 128), 10, "batch"),      # 256 cubes, per-cube parameters
 }
+BATCH = 256
+# reference filters (PAPER.md:402-405 timing parameters); --filter idg is the contract's metric
+FILTERS = {"idg": None, "box": ("box", (3, 3, 3)), "box_aniso": ("box", (3, 5, 5)),
+           "gauss": ("gauss", (3.0, 3.0, 3.0), (0.0, 0.0, 0.0)), "gauss_aniso": ("gauss", (2.0, 3.0, 3.0), (0.0, 0.0, 0.0)),
+           "gauss_rot": ("gauss", (2.0, 3.0, 3.0), (10.0, 20.0, 30.0))}
 DEFAULT_WORKLOAD = "cfg3_1024x1024x512_n20"
 
 
@@ -47,6 +53,8 @@ def make_cube(name: str, seed_offset: int = 0, threads=None):
         c = synth.large_cube(seed=3000 + seed_offset, shape=shape, threads=threads)
     elif gen == "survey":
         c = synth.survey_field(shape, seed=2000 + seed_offset, n_discs=6, threads=threads)
+    elif gen == "batch":                      # one cube of the batch (reference arm / oracle sample)
+        c = synth.modelb_like(shape, seed=4000 + seed_offset, snr=32.0, threads=threads)
     else:
         c = synth.modelb_like(shape, seed=1000 + seed_offset, snr=32.0, threads=threads)
     return c, n
@@ -212,15 +220,32 @@ def run_ours(args) -> None:
     B.idg_set_option(B.IDG_OPT_TILE, args.tile)
 
     threads = max(1, (os.cpu_count() or 1) // max(1, world))
-    cube, n = make_cube(args.workload, seed_offset=rank, threads=threads)
-    nz, ny, nx = cube.data.shape
-    N = nz * ny * nx
+    batched = WORKLOADS[args.workload][2] == "batch"
+    filt = FILTERS[args.filter]
+    if batched:
+        from paper_1609_03782_b200 import synth
+        shape, n, _ = WORKLOADS[args.workload]
+        data = synth.batch_cubes(BATCH, seed=4000 + 1000 * rank, shape=shape, threads=threads)
+        plist = [B.Params(*[float(v) for v in row]) for row in synth.batch_params(BATCH, seed=4000 + 1000 * rank)]
+        nz, ny, nx = shape
+        N = BATCH * nz * ny * nx
+        args.no_e2e = True                    # the host-buffer entry point takes one cube
+    else:
+        cube, n = make_cube(args.workload, seed_offset=rank, threads=threads)
+        data = cube.data
+        nz, ny, nx = data.shape
+        N = nz * ny * nx
     p = B.Params()                            # PAPER.md:187 defaults; rms = 1 by construction
-    host_in = torch.from_numpy(cube.data).pin_memory()
+    host_in = torch.from_numpy(data).pin_memory()
     d_in = host_in.cuda(non_blocking=True)
     d_out = torch.empty_like(d_in)
-    ws = B.alloc_workspace(nx, ny, nz, 1)
+    ws = B.alloc_workspace(nx, ny, nz, BATCH if batched else 1)
     stream = torch.cuda.current_stream()
+    if filt is not None:
+        if batched:
+            raise SystemExit("--filter box/gauss runs on single-cube workloads")
+        n = 1                                 # one pass; throughput in Gvoxel/s
+        args.no_e2e = True
 
     def barrier():
         torch.cuda.synchronize()
@@ -229,7 +254,15 @@ def run_ours(args) -> None:
         torch.cuda.synchronize()
 
     def step():
-        B.idg_filter(d_in, n, p, out=d_out, workspace=ws, stream=stream)
+        if filt is not None:
+            if filt[0] == "box":
+                B.idg_box_filter(d_in, *filt[1], out=d_out, stream=stream)
+            else:
+                B.idg_gaussian_filter(d_in, filt[1], filt[2], out=d_out, stream=stream)
+        elif batched:
+            B.idg_filter_batched(d_in, n, plist, out=d_out, workspace=ws, stream=stream)
+        else:
+            B.idg_filter(d_in, n, p, out=d_out, workspace=ws, stream=stream)
 
     for _ in range(max(3, args.warmup)):
         step()
@@ -278,15 +311,33 @@ def run_ours(args) -> None:
     ms_launch = ms_step / launches_per_step
     achieved = BYTES_PER_VOXEL_ITER * N * fuse / (ms_launch * 1e-3) / 1e9     # algorithmic GB/s per launch
     kernel_tag = f"{plan} {args.workload}"
-    cpu_v, cores, sample, _ = oracle_rate(cube.data, n, 15.0, p.f32())
+    if filt is not None:                      # reference filter: its own metric, oracle timed on a small block
+        import oracle
+        cores = oracle.set_threads(os.cpu_count() or 1)
+        blk = data[:min(nz, 48), :min(ny, 256), :min(nx, 256)]
+        t0 = time.perf_counter()
+        if filt[0] == "box":
+            oracle.box_filter_oracle(blk, *filt[1])
+        else:
+            oracle.gaussian_filter_oracle(blk, filt[1], filt[2])
+        dt = time.perf_counter() - t0
+        cpu_v, sample = blk.size / dt / 1e9, f"{blk.shape[2]}x{blk.shape[1]}x{blk.shape[0]} block, direct 3-D sum, fp64, {dt:.1f} s"
+        metric, unit, params = f"{args.filter}_filter_throughput", "Gvoxel/s", str(filt[1:])
+    else:
+        first = data[0] if batched else data
+        cpu_v, cores, sample, _ = oracle_rate(first, n, 15.0, (plist[0] if batched else p).f32())
+        metric, unit = METRIC, UNIT
+        params = ("per-cube K, tau, C_j (synth.batch_params)" if batched
+                  else "K=1.5 tau=0.0325 Cx=Cy=Cz=5 rms=1 (PAPER.md:187, :406)")
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps,
         "warmup": max(3, args.warmup), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": args.workload, "shape_xyz": [nx, ny, nz], "n_iter": n,
-                   "params": "K=1.5 tau=0.0325 Cx=Cy=Cz=5 rms=1 (PAPER.md:187, :406)",
+                   "params": params, "batch": BATCH if batched else 1,
                    "fused_iterations_per_launch": fuse, "parallelism": f"replicas x{world}",
-                   "l2": "cube (2.1 GB) and scratch exceed the 126 MB L2; no flush needed",
+                   "l2": f"input + output ({2 * N * 4 / 1e6:.0f} MB per call) against the 126 MB L2: "
+                         + ("larger, no flush needed" if 2 * N * 4 > 252e6 else "NOT larger -- warm-L2 number"),
                    "paper_context": "GTX860M OpenGL 0.90, i7 8 threads 0.036 Gvoxel-iter/s (PAPER.md:408-414)"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": ncu_traffic_bytes(kernel_tag),
@@ -295,12 +346,20 @@ def run_ours(args) -> None:
                      "peak_source": peak_src,
                      "note": "algorithmic bytes = 8 B x voxels x fused iterations (what an un-fused sweep must "
                              "move); temporal fusion moves fewer DRAM bytes, so frac can exceed 1 -- see traffic"},
-        "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N * 4, "d2h_bytes_per_step": N * 4,
+        "cpu_baseline": {"value": cpu_v, "unit": unit, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": e2e_value, "unit": unit, "h2d_bytes_per_step": N * 4, "d2h_bytes_per_step": N * 4,
                 "api": "idg_filter_host (pinned host buffers)"},
         "gpu_launches": launches_per_step * args.steps,
         "clocks": clocks,
     }
+    if filt is not None and any(filt[2:] and filt[2]):     # rotated Gaussian: bound by FP32, not by HBM
+        r = B.idg_gaussian_radii(filt[1], filt[2])[0]
+        flops = 2.0 * (2 * r + 1) ** 3 * N
+        peak_tf = 148 * 128 * 2 * 1.965e9 / 1e12          # SMs x FP32 lanes x 2 flop x max clock (B200_PROFILING.md)
+        line["roofline"] = {"bound": "alu", "achieved": flops / (ms_launch * 1e-3) / 1e12, "peak": peak_tf,
+                            "unit": "TFLOP/s", "frac": flops / (ms_launch * 1e-3) / 1e12 / peak_tf, "traffic": None,
+                            "kernel": plan, "ms_per_launch": ms_launch,
+                            "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz"}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -313,6 +372,8 @@ def main() -> None:
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
+    ap.add_argument("--filter", default="idg", choices=sorted(FILTERS),
+                    help="idg (the contract's metric) or a reference filter: one pass, Gvoxel/s")
     ap.add_argument("--fuse", type=int, default=0, help="iterations fused per launch (0 = library default)")
     ap.add_argument("--zchunk", type=int, default=0, help="planes per CTA along z (0 = library default)")
     ap.add_argument("--tile", type=int, default=0, help="TMA kernel tile variant (0 = library default)")
