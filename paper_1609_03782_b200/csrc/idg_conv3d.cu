@@ -3,11 +3,11 @@
 //
 //   out(x,y,z) = sum_{|i|,|j|,|k| <= r} K(i,j,k) I(cx(x+i), cy(y+j), cz(z+k))
 //
-// (K is even, so convolution and correlation coincide.)  A CTA produces a 32 x 8 x 8 block from the
+// (K is even, so convolution and correlation coincide.)  A CTA produces a 32 x 8 x 16 block from the
 // block plus halo staged in shared memory together with the (2r+1)^3 weights.  A thread owns one
-// (x, y) column of 8 outputs along z: for every (i, j) it loads the 8 + 2r inputs of the shifted
-// column and the 2r + 1 weights K(i, j, .) into registers once and issues 8 (2r+1) FMAs on them, so
-// shared-memory traffic is ~1/3 load per FMA and the kernel is bound by the FP32 pipe, as a
+// (x, y) column of 16 outputs along z: for every (i, j) it loads the 16 + 2r inputs of the shifted
+// column and the 2r + 1 weights K(i, j, .) into registers once and issues 16 (2r+1) FMAs on them, so
+// shared-memory traffic is ~1/4 load per FMA and the kernel is bound by the FP32 pipe, as a
 // (2r+1)^3-tap filter should be.  r is a template parameter (register windows).
 #include "idg_kernels.cuh"
 
@@ -15,7 +15,10 @@ namespace idg {
 
 namespace {
 
-constexpr int BX = 32, BY = 8, BZ = 8, NT = 256;
+constexpr int BX = 32, BY = 8, NT = 256;
+// outputs per thread along z: 16 where the halo block still fits shared memory (shared-memory
+// wavefronts per FMA 0.23, FP32-bound), 8 for the two largest radii
+__host__ __device__ constexpr int bz_of(int r) { return r <= 8 ? 16 : 8; }
 
 struct ConvArgs {
     const float *in;
@@ -27,7 +30,7 @@ struct ConvArgs {
 template <int R>
 __global__ void __launch_bounds__(NT) idg_conv3d_kernel(const __grid_constant__ ConvArgs S)
 {
-    constexpr int W = 2 * R + 1;
+    constexpr int W = 2 * R + 1, BZ = bz_of(R);
     constexpr int SX = BX + 2 * R, SY = BY + 2 * R, SZ = BZ + 2 * R;
     extern __shared__ __align__(16) float smem[];
     float *tile = smem;                          // SZ x SY x SX
@@ -75,7 +78,7 @@ __global__ void __launch_bounds__(NT) idg_conv3d_kernel(const __grid_constant__ 
 template <int R>
 cudaError_t launch_r(const ConvArgs &S, cudaStream_t st)
 {
-    constexpr int W = 2 * R + 1;
+    constexpr int W = 2 * R + 1, BZ = bz_of(R);
     constexpr size_t smem = sizeof(float) * ((size_t)(BX + 2 * R) * (BY + 2 * R) * (BZ + 2 * R) + (size_t)W * W * W);
     static_assert(smem <= 227u * 1024u, "shared memory budget");
     static bool attr_done = false;
