@@ -42,7 +42,8 @@ BATCH = 256
 # reference filters (PAPER.md:402-405 timing parameters); --filter idg is the contract's metric
 FILTERS = {"idg": None, "box": ("box", (3, 3, 3)), "box_aniso": ("box", (3, 5, 5)),
            "gauss": ("gauss", (3.0, 3.0, 3.0), (0.0, 0.0, 0.0)), "gauss_aniso": ("gauss", (2.0, 3.0, 3.0), (0.0, 0.0, 0.0)),
-           "gauss_rot": ("gauss", (2.0, 3.0, 3.0), (10.0, 20.0, 30.0))}
+           "gauss_rot": ("gauss", (2.0, 3.0, 3.0), (10.0, 20.0, 30.0)),
+           "mask_sums": ("quality",)}                 # Eq. 13-14 over the whole cube: reads 2 cubes
 DEFAULT_WORKLOAD = "cfg3_1024x1024x512_n20"
 
 
@@ -246,6 +247,9 @@ def run_ours(args) -> None:
             raise SystemExit("--filter box/gauss runs on single-cube workloads")
         n = 1                                 # one pass; throughput in Gvoxel/s
         args.no_e2e = True
+        if filt[0] == "quality":              # the "filtered" cube: a box-smoothed copy
+            B.idg_box_filter(d_in, 3, 3, 3, out=d_out, stream=stream)
+            q_sums = torch.empty(8, dtype=torch.float64, device="cuda")
 
     def barrier():
         torch.cuda.synchronize()
@@ -255,7 +259,9 @@ def run_ours(args) -> None:
 
     def step():
         if filt is not None:
-            if filt[0] == "box":
+            if filt[0] == "quality":
+                B.idg_mask_sums(d_in, d_out, None, 3.0, 1.5, None, sums=q_sums, stream=stream)
+            elif filt[0] == "box":
                 B.idg_box_filter(d_in, *filt[1], out=d_out, stream=stream)
             else:
                 B.idg_gaussian_filter(d_in, filt[1], filt[2], out=d_out, stream=stream)
@@ -316,13 +322,18 @@ def run_ours(args) -> None:
         cores = oracle.set_threads(os.cpu_count() or 1)
         blk = data[:min(nz, 48), :min(ny, 256), :min(nx, 256)]
         t0 = time.perf_counter()
-        if filt[0] == "box":
+        if filt[0] == "quality":
+            from oracle import quality_oracle
+            blk = data
+            t0 = time.perf_counter()
+            quality_oracle.mask_sums_oracle(blk, blk, None, 3.0, 1.5)
+        elif filt[0] == "box":
             oracle.box_filter_oracle(blk, *filt[1])
         else:
             oracle.gaussian_filter_oracle(blk, filt[1], filt[2])
         dt = time.perf_counter() - t0
-        cpu_v, sample = blk.size / dt / 1e9, f"{blk.shape[2]}x{blk.shape[1]}x{blk.shape[0]} block, direct 3-D sum, fp64, {dt:.1f} s"
-        metric, unit, params = f"{args.filter}_filter_throughput", "Gvoxel/s", str(filt[1:])
+        cpu_v, sample = blk.size / dt / 1e9, f"{blk.shape[2]}x{blk.shape[1]}x{blk.shape[0]} block, oracle as it stands, fp64, {dt:.1f} s"
+        metric, unit, params = f"{args.filter}_throughput", "Gvoxel/s", str(filt[1:])
     else:
         first = data[0] if batched else data
         cpu_v, cores, sample, _ = oracle_rate(first, n, 15.0, (plist[0] if batched else p).f32())
@@ -352,7 +363,7 @@ def run_ours(args) -> None:
         "gpu_launches": launches_per_step * args.steps,
         "clocks": clocks,
     }
-    if filt is not None and any(filt[2:] and filt[2]):     # rotated Gaussian: bound by FP32, not by HBM
+    if filt is not None and len(filt) > 2 and any(filt[2]):     # rotated Gaussian: bound by FP32, not by HBM
         r = B.idg_gaussian_radii(filt[1], filt[2])[0]
         flops = 2.0 * (2 * r + 1) ** 3 * N
         peak_tf = 148 * 128 * 2 * 1.965e9 / 1e12          # SMs x FP32 lanes x 2 flop x max clock (B200_PROFILING.md)

@@ -164,6 +164,42 @@ int idg_gaussian_radii(float fwhm_x, float fwhm_y, float fwhm_z, float theta_x, 
                        int radii[3]);
 
 /*
+ * Smoothing-quality diagnostics (Eq. 12-16; Eq. 17-18).
+ * A region of interest is the half-open index box [x0,x1) x [y0,y1) x [z0,z1) (NULL = whole cube).
+ */
+typedef struct idg_roi { int x0, x1, y0, y1, z0, z1; } idg_roi;
+
+/*
+ * One pass over the original, the filtered and (optionally) the noiseless model cube:
+ *   M_o = [I_o >= thr_o], M_f = [I_f >= thr_f]   (Eq. 14 with thr_i = 3 rms_i; fp32 compare, NaN never passes)
+ *   sums[0] = S_oo = sum I_o M_o     sums[1] = S_of = sum I_o M_f      (Eq. 13)
+ *   sums[2] = N_o  = sum M_o         sums[3] = N_f  = sum M_f          (Eq. 16)
+ *   sums[4] = S_mf = sum I_m M_f     sums[5] = S_m  = sum I_m          (Eq. 18; 0 when model is NULL)
+ *   sums[6] = voxels in the ROI      sums[7] = 0
+ * over the ROI, accumulated in fp64 (counts are exact).
+ *   orig, filt, model [device] nx*ny*nz fp32 (model may be NULL);  roi [host] or NULL
+ *   sums [device] 8 doubles, 8-byte aligned; overwritten.  Errors: IDG_ERR_DIMS for a ROI outside the
+ *   cube, IDG_ERR_PARAM for a NaN threshold, IDG_ERR_WORKSPACE for a misaligned `sums`.
+ */
+int idg_mask_sums(const float *orig, const float *filt, const float *model, int nx, int ny, int nz,
+                  const idg_roi *roi, float thr_o, float thr_f, double *sums, void *stream);
+
+/*
+ * stats[0] = n, stats[1] = sum, stats[2] = sum of squares of the voxels of the ROI (fp64); the noise
+ * level of a signal-free ROI is sqrt(stats[2]/n - (stats[1]/n)^2) (reading Q4).
+ *   cube [device];  stats [device] 8 doubles, 8-byte aligned; overwritten
+ */
+int idg_cube_stats(const float *cube, int nx, int ny, int nz, const idg_roi *roi, double *stats, void *stream);
+
+/*
+ * Host-only: F = |S_of|/|S_oo| (Eq. 12), its error (Eq. 15-16, with N_i = population / voxels_per_beam,
+ * voxels_per_beam >= 1) and F_M = |S_mf|/|S_m| (Eq. 17) from a HOST copy of the sums.  Any of the three
+ * output pointers may be NULL; a ratio with a zero denominator is NaN.
+ */
+int idg_quality(const double *sums, double rms_o, double rms_f, double voxels_per_beam, double *F, double *sigma_F,
+                double *F_M);
+
+/*
  * Process-wide tuning knobs (tests and benchmarks; defaults give the fastest plan).
  *   IDG_OPT_KERNEL   0 auto | 1 naive (one thread per voxel) | 2 tiled z-streaming kernel (global loads)
  *                    | 3 tiled z-streaming kernel fed by TMA | 4 persistent warp-decoupled TMA kernel

@@ -24,7 +24,8 @@ KERNEL_AUTO, KERNEL_NAIVE, KERNEL_TILED, KERNEL_TMA, KERNEL_STREAM = 0, 1, 2, 3,
 SYMBOLS = ("idg_version", "idg_status_string", "idg_params_check", "idg_workspace_bytes",
            "idg_filter", "idg_filter_ws", "idg_filter_batched", "idg_filter_host",
            "idg_set_option", "idg_get_option", "idg_last_launch_count", "idg_last_plan",
-           "idg_box_filter", "idg_gaussian_filter", "idg_gaussian_radii")
+           "idg_box_filter", "idg_gaussian_filter", "idg_gaussian_radii",
+           "idg_mask_sums", "idg_cube_stats", "idg_quality")
 
 
 class IdgParams(ctypes.Structure):
@@ -49,6 +50,11 @@ class Params:
     def f32(self) -> dict:
         """The fp32-rounded values the library sees, as Python floats (for the oracle)."""
         return {k: float(np.float32(getattr(self, k))) for k in ("K", "tau", "cx", "cy", "cz", "rms")}
+
+
+class IdgRoi(ctypes.Structure):
+    """struct idg_roi: half-open index box [x0,x1) x [y0,y1) x [z0,z1)."""
+    _fields_ = [(n, ctypes.c_int) for n in ("x0", "x1", "y0", "y1", "z0", "z1")]
 
 
 class IdgError(RuntimeError):
@@ -98,6 +104,13 @@ def lib() -> ctypes.CDLL:
         L.idg_gaussian_filter.argtypes = [fp, i, i, i, f, f, f, f, f, f, fp, vp]
         L.idg_gaussian_radii.restype = i
         L.idg_gaussian_radii.argtypes = [f, f, f, f, f, f, ctypes.POINTER(ctypes.c_int)]
+        rp, d, dptr = ctypes.POINTER(IdgRoi), ctypes.c_double, ctypes.POINTER(ctypes.c_double)
+        L.idg_mask_sums.restype = i
+        L.idg_mask_sums.argtypes = [fp, fp, fp, i, i, i, rp, f, f, vp, vp]
+        L.idg_cube_stats.restype = i
+        L.idg_cube_stats.argtypes = [fp, i, i, i, rp, vp, vp]
+        L.idg_quality.restype = i
+        L.idg_quality.argtypes = [dptr, d, d, d, dptr, dptr, dptr]
         _lib = L
     return _lib
 
@@ -257,6 +270,52 @@ def idg_gaussian_radii(fwhm: Sequence[float], theta: Sequence[float] = (0.0, 0.0
     _check(lib().idg_gaussian_radii(float(fwhm[0]), float(fwhm[1]), float(fwhm[2]), float(theta[0]),
                                     float(theta[1]), float(theta[2]), r))
     return int(r[0]), int(r[1]), int(r[2])
+
+
+def _roi(roi) -> Optional[IdgRoi]:
+    return None if roi is None else IdgRoi(*[int(v) for v in roi])
+
+
+SUM_KEYS = ("S_oo", "S_of", "N_o", "N_f", "S_mf", "S_m", "n_roi")
+
+
+def idg_mask_sums(orig: torch.Tensor, filt: torch.Tensor, model: Optional[torch.Tensor], thr_o: float,
+                  thr_f: float, roi=None, sums: Optional[torch.Tensor] = None,
+                  stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """idg_mask_sums on [nz, ny, nx] CUDA tensors; roi = (x0, x1, y0, y1, z0, z1) or None.
+    Returns the device tensor of 8 doubles (asynchronous on `stream`)."""
+    nz, ny, nx = orig.shape
+    if filt.shape != orig.shape or (model is not None and model.shape != orig.shape):
+        raise ValueError("cubes must have equal shapes")
+    if sums is None:
+        sums = torch.empty(8, dtype=torch.float64, device=orig.device)
+    r = _roi(roi)
+    _check(lib().idg_mask_sums(_dev(orig, "orig"), _dev(filt, "filt"),
+                               None if model is None else _dev(model, "model"), nx, ny, nz,
+                               None if r is None else ctypes.byref(r), float(thr_o), float(thr_f),
+                               sums.data_ptr(), _stream(stream)))
+    return sums
+
+
+def idg_cube_stats(cube: torch.Tensor, roi=None, stats: Optional[torch.Tensor] = None,
+                   stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """idg_cube_stats: device tensor of 8 doubles (n, sum, sum of squares, 0...)."""
+    nz, ny, nx = cube.shape
+    if stats is None:
+        stats = torch.empty(8, dtype=torch.float64, device=cube.device)
+    r = _roi(roi)
+    _check(lib().idg_cube_stats(_dev(cube, "cube"), nx, ny, nz, None if r is None else ctypes.byref(r),
+                                stats.data_ptr(), _stream(stream)))
+    return stats
+
+
+def idg_quality(sums: Sequence[float], rms_o: float, rms_f: float, voxels_per_beam: float = 1.0) -> dict:
+    """idg_quality on a HOST copy of the sums: {"F", "sigma_F", "F_M"} (Eq. 12, 15-17)."""
+    arr = (ctypes.c_double * 8)(*[float(v) for v in list(sums)[:8]] + [0.0] * (8 - min(8, len(sums))))
+    out = [ctypes.c_double() for _ in range(3)]
+    _check(lib().idg_quality(arr, float(rms_o), float(rms_f), float(voxels_per_beam),
+                             *[ctypes.byref(o) for o in out]))
+    return {"F": out[0].value, "sigma_F": out[1].value, "F_M": out[2].value}
 
 
 def host_buffers_bytes(nx: int, ny: int, nz: int) -> int:

@@ -431,6 +431,71 @@ int idg_gaussian_filter(const float *cube, int nx, int ny, int nz, float fwhm_x,
     return IDG_OK;
 }
 
+// ---- quality diagnostics (section 4-5, Eq. 12-18) ------------------------------------
+
+static int roi_box(const idg_roi *roi, int nx, int ny, int nz, int r[6])
+{
+    if (!roi) { r[0] = 0; r[1] = nx; r[2] = 0; r[3] = ny; r[4] = 0; r[5] = nz; return IDG_OK; }
+    r[0] = roi->x0; r[1] = roi->x1; r[2] = roi->y0; r[3] = roi->y1; r[4] = roi->z0; r[5] = roi->z1;
+    if (r[0] < 0 || r[0] > r[1] || r[1] > nx || r[2] < 0 || r[2] > r[3] || r[3] > ny || r[4] < 0 || r[4] > r[5] ||
+        r[5] > nz)
+        return IDG_ERR_DIMS;
+    return IDG_OK;
+}
+
+int idg_mask_sums(const float *orig, const float *filt, const float *model, int nx, int ny, int nz,
+                  const idg_roi *roi, float thr_o, float thr_f, double *sums, void *stream)
+{
+    t_launches = 0;
+    if (!orig || !filt || !sums) return IDG_ERR_NULL;
+    size_t N;
+    if (!voxel_count(nx, ny, nz, 1, &N)) return IDG_ERR_DIMS;
+    if (isnan(thr_o) || isnan(thr_f)) return IDG_ERR_PARAM;
+    if (((uintptr_t)sums & 7u) != 0) return IDG_ERR_WORKSPACE;
+    int r[6];
+    const int rc = roi_box(roi, nx, ny, nz, r);
+    if (rc != IDG_OK) return rc;
+    const cudaError_t e = idg::launch_mask_sums(orig, filt, model, nx, ny, r, thr_o, thr_f, sums, (cudaStream_t)stream);
+    if (e != cudaSuccess) return (int)e;
+    t_launches = 1;
+    snprintf(t_plan, sizeof(t_plan), "idg_mask_sums_kernel<model=%d>", model ? 1 : 0);
+    return IDG_OK;
+}
+
+int idg_cube_stats(const float *cube, int nx, int ny, int nz, const idg_roi *roi, double *stats, void *stream)
+{
+    t_launches = 0;
+    if (!cube || !stats) return IDG_ERR_NULL;
+    size_t N;
+    if (!voxel_count(nx, ny, nz, 1, &N)) return IDG_ERR_DIMS;
+    if (((uintptr_t)stats & 7u) != 0) return IDG_ERR_WORKSPACE;
+    int r[6];
+    const int rc = roi_box(roi, nx, ny, nz, r);
+    if (rc != IDG_OK) return rc;
+    const cudaError_t e = idg::launch_cube_stats(cube, nx, ny, r, stats, (cudaStream_t)stream);
+    if (e != cudaSuccess) return (int)e;
+    t_launches = 1;
+    snprintf(t_plan, sizeof(t_plan), "idg_cube_stats_kernel");
+    return IDG_OK;
+}
+
+int idg_quality(const double *sums, double rms_o, double rms_f, double voxels_per_beam, double *F, double *sigma_F,
+                double *F_M)
+{
+    if (!sums) return IDG_ERR_NULL;
+    if (!(rms_o > 0.0) || !(rms_f > 0.0) || !(voxels_per_beam >= 1.0)) return IDG_ERR_PARAM;
+    const double S_oo = sums[0], S_of = sums[1], N_o = sums[2], N_f = sums[3], S_mf = sums[4], S_m = sums[5];
+    const double nan = NAN;
+    if (F) *F = S_oo != 0.0 ? fabs(S_of) / fabs(S_oo) : nan;                                     // Eq. 12
+    if (sigma_F) {
+        const double sig_of = sqrt(N_f / voxels_per_beam) * rms_f, sig_oo = sqrt(N_o / voxels_per_beam) * rms_o;   // Eq. 16
+        *sigma_F = S_oo != 0.0 ? sqrt(sig_of * sig_of / (S_oo * S_oo) +
+                                      S_of * S_of * sig_oo * sig_oo / (S_oo * S_oo * S_oo * S_oo)) : nan;          // Eq. 15
+    }
+    if (F_M) *F_M = S_m != 0.0 ? fabs(S_mf) / fabs(S_m) : nan;                                   // Eq. 17
+    return IDG_OK;
+}
+
 int idg_set_option(int key, int value)
 {
     if (key < 0 || key >= IDG_OPT_COUNT_) return IDG_ERR_OPTION;

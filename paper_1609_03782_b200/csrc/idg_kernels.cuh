@@ -97,4 +97,10 @@ cudaError_t launch_sep3d(const float *in, float *out, int nx, int ny, int nz, in
 cudaError_t launch_conv3d(const float *in, float *out, int nx, int ny, int nz, int r, const float *kern,
                           cudaStream_t st);
 
+
+// Quality diagnostics (Eq. 12-18): masked sums and cube statistics over a ROI, 8 doubles out.
+cudaError_t launch_mask_sums(const float *o, const float *f, const float *m, int nx, int ny, const int roi[6],
+                             float thr_o, float thr_f, double *out, cudaStream_t st);
+cudaError_t launch_cube_stats(const float *cube, int nx, int ny, const int roi[6], double *out, cudaStream_t st);
+
 }  // namespace idg
