@@ -350,3 +350,30 @@ def test_launch_count(B):
         set_plan(B, (k, 2))
         B.idg_filter(t, 7)
         assert B.idg_last_launch_count() == 4
+
+
+@pytest.mark.parametrize("plan", [(2, 2), (3, 1), (3, 2), (3, 3), (3, 4), (4, 1), (4, 2), (4, 3), (4, 4)],
+                         ids=lambda p: f"k{p[0]}-T{p[1]}")
+def test_fused_kernels_are_bitwise_equal_to_the_naive_kernel_and_repeatable(B, plan):
+    """Every kernel applies the same fp32 operations in the same order per voxel (packed fp32x2
+    arithmetic rounds like the scalar update), so any fusion depth, tiling and grid must reproduce
+    the one-thread-per-voxel kernel bit for bit -- and do so on every run: a synchronisation race in
+    the barrier-free plane loop (mbarriers, stage hand-back) would show up as a differing voxel."""
+    g = torch.Generator(device="cuda").manual_seed(99)
+    x = torch.randn((40, 300, 520), device="cuda", generator=g) * 2.0
+    p = B.Params(K=1.5, tau=0.03, cx=5.0, cy=4.0, cz=6.0, rms=1.0)
+    set_plan(B, (1, 0))
+    ref = B.idg_filter(x, 7, p)
+    for tile in ((1, 2) if plan[0] >= 3 and plan[1] <= 2 else (0,)):
+        for rep in range(4):
+            set_plan(B, plan, 0, tile)
+            out = B.idg_filter(x, 7, p)
+            torch.cuda.synchronize()
+            assert torch.equal(out, ref), (plan, tile, rep, int((out != ref).sum()))
+    xb = torch.randn((12, 20, 64, 128), device="cuda", generator=g)
+    set_plan(B, (1, 0))
+    refb = B.idg_filter_batched(xb, [5, 3, 7, 0, 1, 6, 2, 7, 4, 5, 3, 7], [p] * 12)
+    set_plan(B, plan)
+    for rep in range(3):
+        outb = B.idg_filter_batched(xb, [5, 3, 7, 0, 1, 6, 2, 7, 4, 5, 3, 7], [p] * 12)
+        assert torch.equal(outb, refb), (plan, rep)
