@@ -48,6 +48,8 @@ def _load() -> ctypes.CDLL:
                                        ctypes.c_double, ctypes.c_double, ctypes.c_double, dp, dp]
         lib.idg_oracle_set_threads.restype = ctypes.c_int
         lib.idg_oracle_set_threads.argtypes = [ctypes.c_int]
+        lib.pm_oracle_f64.restype = ctypes.c_int
+        lib.pm_oracle_f64.argtypes = lib.idg_oracle_f64.argtypes
         ip = ctypes.POINTER(ctypes.c_int)
         lib.box_oracle_f64.restype = ctypes.c_int
         lib.box_oracle_f64.argtypes = [dp] + [ctypes.c_int] * 6 + [dp]
@@ -88,6 +90,24 @@ def idg_filter_oracle(cube: np.ndarray, n_iter: int, K: float = 1.5, tau: float 
                                 float(rms), out.ctypes.data_as(dp), scratch.ctypes.data_as(dp))
     if rc != 0:
         raise ValueError(f"idg_oracle_f64 rejected its arguments (rc={rc})")
+    return out
+
+
+def pm_filter_oracle(cube: np.ndarray, n_iter: int, K: float = 1.5, tau: float = 0.0325,
+                     cx: float = 5.0, cy: float = 5.0, cz: float = 5.0, rms: float = 1.0) -> np.ndarray:
+    """n_iter updates of the gradient-driven (Perona-Malik, Eq. 5) variant of Eq. 7 in fp64:
+    conductance 1/(1 + |grad I|^2/(K^2 rms^2)) from central differences of the six neighbours."""
+    a = np.ascontiguousarray(cube, dtype=np.float64)
+    if a.ndim != 3:
+        raise ValueError("cube must be 3-D [nz, ny, nx]")
+    nz, ny, nx = a.shape
+    out, scratch = np.empty_like(a), np.empty_like(a)
+    dp = ctypes.POINTER(ctypes.c_double)
+    rc = _load().pm_oracle_f64(a.ctypes.data_as(dp), nx, ny, nz, int(n_iter), float(K), float(tau),
+                               float(cx), float(cy), float(cz), float(rms), out.ctypes.data_as(dp),
+                               scratch.ctypes.data_as(dp))
+    if rc != 0:
+        raise ValueError(f"pm_oracle_f64 rejected its arguments (rc={rc})")
     return out
 
 
