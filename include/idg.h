@@ -105,6 +105,16 @@ int idg_filter_ws(const float *cube, int nx, int ny, int nz, int n_iter,
                   void *workspace, size_t workspace_bytes, void *stream);
 
 /*
+ * Gradient-driven variant: as idg_filter_ws, but the conductance of Eq. 7 is the classic Perona-Malik
+ * one (Eq. 5), S = 1 / (1 + |grad I_i|^2 / (K^2 rms^2)), with |grad I|^2 the sum over
+ * the axes of the squared central difference [I(+1) - I(-1)] / 2 of the same six neighbours
+ * (replicated faces; K in units of rms per voxel: DESIGN.md readings P1-P3).  K = +INFINITY gives the
+ * same linear diffusion as idg_filter.
+ */
+int idg_filter_pm(const float *cube, int nx, int ny, int nz, int n_iter, const idg_params *params,
+                  float *out, void *workspace, size_t workspace_bytes, void *stream);
+
+/*
  * `batch` independent cubes of equal shape in one call (interactive parameter
  * exploration), each with its own parameters and
  * iteration count.

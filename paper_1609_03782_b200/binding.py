@@ -25,7 +25,7 @@ SYMBOLS = ("idg_version", "idg_status_string", "idg_params_check", "idg_workspac
            "idg_filter", "idg_filter_ws", "idg_filter_batched", "idg_filter_host",
            "idg_set_option", "idg_get_option", "idg_last_launch_count", "idg_last_plan",
            "idg_box_filter", "idg_gaussian_filter", "idg_gaussian_radii",
-           "idg_mask_sums", "idg_cube_stats", "idg_quality")
+           "idg_mask_sums", "idg_cube_stats", "idg_quality", "idg_filter_pm")
 
 
 class IdgParams(ctypes.Structure):
@@ -87,6 +87,8 @@ def lib() -> ctypes.CDLL:
         L.idg_filter.argtypes = [fp, i, i, i, i, pp, fp, vp]
         L.idg_filter_ws.restype = i
         L.idg_filter_ws.argtypes = [fp, i, i, i, i, pp, fp, vp, sz, vp]
+        L.idg_filter_pm.restype = i
+        L.idg_filter_pm.argtypes = [fp, i, i, i, i, pp, fp, vp, sz, vp]
         L.idg_filter_batched.restype = i
         L.idg_filter_batched.argtypes = [fp, i, i, i, i, ip, i, pp, fp, vp, sz, vp]
         L.idg_filter_host.restype = i
@@ -187,6 +189,23 @@ def idg_filter(cube: torch.Tensor, n_iter: int, params: Params = Params(),
                                  _dev(out, "out"), workspace.data_ptr(), workspace.numel(),
                                  _stream(stream))
     _check(rc)
+    return out
+
+
+def idg_filter_pm(cube: torch.Tensor, n_iter: int, params: Params = Params(),
+                  out: Optional[torch.Tensor] = None, workspace: Optional[torch.Tensor] = None,
+                  stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """idg_filter_pm (gradient-driven conductance, Eq. 5) on a [nz, ny, nx] CUDA tensor."""
+    if cube.dim() != 3:
+        raise ValueError("cube must be [nz, ny, nx]")
+    nz, ny, nx = cube.shape
+    if out is None:
+        out = torch.empty_like(cube)
+    if workspace is None:
+        workspace = alloc_workspace(nx, ny, nz, 1, cube.device)
+    c = params.c()
+    _check(lib().idg_filter_pm(_dev(cube, "cube"), nx, ny, nz, int(n_iter), ctypes.byref(c), _dev(out, "out"),
+                               workspace.data_ptr(), workspace.numel(), _stream(stream)))
     return out
 
 

@@ -61,7 +61,7 @@ bool ranges_overlap(const void *a, size_t na, const void *b, size_t nb)
 
 int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter, int n_iter_all,
         const idg_params *params, float *out, void *workspace, size_t workspace_bytes,
-        cudaStream_t st)
+        cudaStream_t st, int mode = 0)
 {
     t_launches = 0;
     if (!cubes || !out || !params) return IDG_ERR_NULL;
@@ -114,6 +114,12 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
             kernel = can_tile ? 2 : 1;
         }
     }
+    if (mode == 1) {          // gradient-driven variant: persistent kernel (T <= 2) or the naive kernel
+        kernel = (can_stream && g_opt[IDG_OPT_KERNEL] != 1) ? 4 : 1;
+        if (fuse > 2 || fuse == 0) fuse = 2;
+        tile = g_opt[IDG_OPT_TILE];
+        if (tile > 2 || tile == 0) tile = ((double)N * (double)batch < 6.4e7) ? 2 : 1;
+    }
     if (kernel == 4 && !can_stream) kernel = 2;
     if (kernel == 3 && !can_tma) kernel = 2;
     if (kernel == 2 && !can_tile) kernel = 1;
@@ -128,7 +134,7 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     {
         static const char *const names[5] = {"", "idg_naive_kernel", "idg_tiled_kernel", "idg_tma_kernel",
                                              "idg_stream_kernel"};
-        snprintf(t_plan, sizeof(t_plan), "%s fuse=%d tile=%d", names[kernel], fuse, tile);
+        snprintf(t_plan, sizeof(t_plan), "%s%s fuse=%d tile=%d", names[kernel], mode == 1 ? " pm" : "", fuse, tile);
     }
 
     std::vector<idg::CubeParams> host_tab((size_t)batch);
@@ -163,6 +169,7 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     L.nx = nx; L.ny = ny; L.nz = nz; L.batch = batch;
     L.fuse = fuse;
     L.in_place = in_place ? 1 : 0;
+    L.mode = mode;
     if (batch == 1) {
         L.tab = nullptr;
         L.one = host_tab[0];
@@ -233,6 +240,13 @@ int idg_filter_ws(const float *cube, int nx, int ny, int nz, int n_iter, const i
 {
     return run(cube, nx, ny, nz, 1, nullptr, n_iter, params, out, workspace, workspace_bytes,
                (cudaStream_t)stream);
+}
+
+int idg_filter_pm(const float *cube, int nx, int ny, int nz, int n_iter, const idg_params *params,
+                  float *out, void *workspace, size_t workspace_bytes, void *stream)
+{
+    return run(cube, nx, ny, nz, 1, nullptr, n_iter, params, out, workspace, workspace_bytes,
+               (cudaStream_t)stream, 1);
 }
 
 int idg_filter_batched(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter,

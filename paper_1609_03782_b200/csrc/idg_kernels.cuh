@@ -28,6 +28,7 @@ struct Launch {
     int iter_done;          // iterations already applied to every cube by earlier launches
     int fuse;               // iterations per launch of this plan (T)
     int in_place;           // out == in: the host staged a copy of I_0 in `scratch`
+    int mode;               // 0: intensity-driven conductance (Eq. 6); 1: gradient-driven (Eq. 5, idg_filter_pm)
 };
 
 // Which buffers cube b reads / writes in this launch so that its LAST launch writes `out`.
@@ -75,6 +76,23 @@ __device__ __forceinline__ float update(float c, float xm, float xp, float ym, f
     const float dz = fmaf(-2.0f, c, zp + zm);
     const float lap = fmaf(az, dz, fmaf(ay, dy, ax * dx));
     return fmaf(lap, conductance(c, s), c);
+}
+
+// Gradient-driven variant of update(): conductance 1/(1 + |grad I|^2 s^2) with central differences
+// (Eq. 5; readings P1-P3).  Same operation order as update2_pm() of idg_stream.cu.
+__device__ __forceinline__ float update_pm(float c, float xm, float xp, float ym, float yp,
+                                           float zm, float zp, float ax, float ay, float az, float s)
+{
+    const float dx = fmaf(-2.0f, c, xp + xm);
+    const float dy = fmaf(-2.0f, c, yp + ym);
+    const float dz = fmaf(-2.0f, c, zp + zm);
+    const float lap = fmaf(az, dz, fmaf(ay, dy, ax * dx));
+    const float gx = xp - xm, gy = fmaf(-1.0f, ym, yp), gz = fmaf(-1.0f, zm, zp);
+    const float G = fmaf(gz, gz, fmaf(gy, gy, gx * gx));
+    const float den = fmaf(0.25f * s * s, G, 1.0f);
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(den));
+    return fmaf(lap, r, c);
 }
 
 // Kernel launchers (each returns cudaGetLastError of its launch).

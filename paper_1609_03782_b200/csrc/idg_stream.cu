@@ -81,9 +81,35 @@ __device__ __forceinline__ float2 update2(float2 c, float2 sx, float2 ym, float2
     const float2 r = make_float2(rcp_approx(den.x), rcp_approx(den.y));
     return __ffma2_rn(lap, r, c);
 }
+// Gradient-driven variant (Eq. 5; readings P1-P3): the conductance is
+// 1/(1 + q G), G = sum_j (I_{+j} - I_{-j})^2, q = s^2/4 (kept in k.s).  gx = difference of the x neighbours.
+__device__ __forceinline__ float2 update2_pm(float2 c, float2 sx, float2 gx, float2 ym, float2 yp, float2 zm,
+                                             float2 zp, const Consts &k)
+{
+    const float2 neg = make_float2(-1.0f, -1.0f);
+    const float2 dx = __ffma2_rn(k.m2, c, sx);
+    const float2 dy = __ffma2_rn(k.m2, c, __fadd2_rn(yp, ym));
+    const float2 dz = __ffma2_rn(k.m2, c, __fadd2_rn(zp, zm));
+    const float2 lap = __ffma2_rn(k.az, dz, __ffma2_rn(k.ay, dy, __fmul2_rn(k.ax, dx)));
+    const float2 gy = __ffma2_rn(neg, ym, yp), gz = __ffma2_rn(neg, zm, zp);
+    const float2 G = __ffma2_rn(gz, gz, __ffma2_rn(gy, gy, __fmul2_rn(gx, gx)));
+    const float2 den = __ffma2_rn(k.s, G, k.one);
+    const float2 r = make_float2(rcp_approx(den.x), rcp_approx(den.y));
+    return __ffma2_rn(lap, r, c);
+}
+template <bool PM>
 __device__ __forceinline__ F4 update4(const F4 &c, float left, float right, const F4 &ym, const F4 &yp,
                                       const F4 &zm, const F4 &zp, const Consts &k)
 {
+    if (PM) {
+        const float2 sx01 = make_float2(c.y + left, c.z + c.x), sx23 = make_float2(c.w + c.y, right + c.z);
+        const float2 gx01 = make_float2(c.y - left, c.z - c.x), gx23 = make_float2(c.w - c.y, right - c.z);
+        const float2 o01 = update2_pm(make_float2(c.x, c.y), sx01, gx01, make_float2(ym.x, ym.y), make_float2(yp.x, yp.y),
+                                      make_float2(zm.x, zm.y), make_float2(zp.x, zp.y), k);
+        const float2 o23 = update2_pm(make_float2(c.z, c.w), sx23, gx23, make_float2(ym.z, ym.w), make_float2(yp.z, yp.w),
+                                      make_float2(zm.z, zm.w), make_float2(zp.z, zp.w), k);
+        return F4{o01.x, o01.y, o23.x, o23.y};
+    }
     const float2 sx01 = make_float2(c.y + left, c.z + c.x);
     const float2 sx23 = make_float2(c.w + c.y, right + c.z);
     const float2 o01 = update2(make_float2(c.x, c.y), sx01, make_float2(ym.x, ym.y), make_float2(yp.x, yp.y),
@@ -254,7 +280,7 @@ struct Pipe {
 
 // One run: `count` consecutive row-planes starting at plane z0 of tile row `tile`, whose cubes all
 // take TL iterations in this launch.
-template <int TL, int R, int WARPS, int NS, int TMAX>
+template <int TL, int R, int WARPS, int NS, int TMAX, bool PM>
 __device__ __forceinline__ void run(const Launch &L, const StreamArgs &A, const Maps &M, unsigned tile, int z0,
                                     unsigned count, Pipe &P, uint32_t sbase)
 {
@@ -318,7 +344,7 @@ __device__ __forceinline__ void run(const Launch &L, const StreamArgs &A, const 
         const uint32_t a0 = sbase + s0 * Y::kStage + S.xo, a1 = sbase + s1 * Y::kStage + S.xo,
                        a2 = sbase + s2 * Y::kStage + S.xo;
         const bool first = (S.ok >> 28) & 1u, last = (S.ok >> 29) & 1u;
-        const Consts kc = make_consts(S.ax, S.ay, S.az, S.sc);
+        const Consts kc = make_consts(S.ax, S.ay, S.az, PM ? 0.25f * S.sc * S.sc : S.sc);
         const bool st_on = cur.q >= cur.qs;
         S.po += plane;
 
@@ -333,7 +359,7 @@ __device__ __forceinline__ void run(const Launch &L, const StreamArgs &A, const 
             float right = __shfl_down_sync(0xffffffffu, c.x, 1);
             left = first ? c.x : left;
             right = last ? c.w : right;
-            const F4 o = update4(c, left, right, pm[r], pm[r + 2], zmv, nwv, kc);
+            const F4 o = update4<PM>(c, left, right, pm[r], pm[r + 2], zmv, nwv, kc);
             if (TL > 1) nw[0][r] = o;                       // level-1 plane q-1
             else if (st_on && (S.ok & (1u << r))) stg128(S.po + (long long)r * L.nx, o.x, o.y, o.z, o.w);
         }
@@ -382,7 +408,7 @@ __device__ __forceinline__ void run(const Launch &L, const StreamArgs &A, const 
                 right = last ? c.w : right;
                 const F4 &ym = (r == 0) ? up : cc[t - 1][r - 1];
                 const F4 &yp = (r == R - 1) ? dn : cc[t - 1][r + 1];
-                const F4 o = update4(c, left, right, ym, yp, zm[t - 1][r], nw[t - 1][r], kc);
+                const F4 o = update4<PM>(c, left, right, ym, yp, zm[t - 1][r], nw[t - 1][r], kc);
                 if (t + 1 < TL) nw[t][r] = o;
                 else if (st_on && (S.ok & (1u << r))) stg128(S.po + (long long)r * L.nx, o.x, o.y, o.z, o.w);
             }
@@ -420,7 +446,7 @@ __device__ __forceinline__ int now_of(const Launch &L, int b)
     return remaining <= 0 ? 0 : (remaining < L.fuse ? remaining : L.fuse);
 }
 
-template <int T, int R, int WARPS, int NS, int MINB>
+template <int T, int R, int WARPS, int NS, int MINB, bool PM>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 idg_stream_kernel(const __grid_constant__ Launch L, const __grid_constant__ StreamArgs A,
                   const __grid_constant__ Maps M)
@@ -459,10 +485,10 @@ idg_stream_kernel(const __grid_constant__ Launch L, const __grid_constant__ Stre
         if (ge > g1) ge = g1;
         const unsigned tile = g / (unsigned)L.nz;
         const int z0 = (int)(g - tile * (unsigned)L.nz);
-        if (now == T) run<T, R, WARPS, NS, T>(L, A, M, tile, z0, ge - g, P, sbase);
-        else if (T > 1 && now == 1) run<1, R, WARPS, NS, T>(L, A, M, tile, z0, ge - g, P, sbase);
-        else if (T > 2 && now == 2) run<(T > 2 ? 2 : 1), R, WARPS, NS, T>(L, A, M, tile, z0, ge - g, P, sbase);
-        else if (T > 3 && now == 3) run<(T > 3 ? 3 : 1), R, WARPS, NS, T>(L, A, M, tile, z0, ge - g, P, sbase);
+        if (now == T) run<T, R, WARPS, NS, T, PM>(L, A, M, tile, z0, ge - g, P, sbase);
+        else if (T > 1 && now == 1) run<1, R, WARPS, NS, T, PM>(L, A, M, tile, z0, ge - g, P, sbase);
+        else if (T > 2 && now == 2) run<(T > 2 ? 2 : 1), R, WARPS, NS, T, PM>(L, A, M, tile, z0, ge - g, P, sbase);
+        else if (T > 3 && now == 3) run<(T > 3 ? 3 : 1), R, WARPS, NS, T, PM>(L, A, M, tile, z0, ge - g, P, sbase);
         __syncthreads();          // drain: every stage is free again before the next run's prologue
         g = ge;
     }
@@ -514,7 +540,7 @@ int sm_count()
     return n;
 }
 
-template <int T, int R, int WARPS, int NS, int MINB>
+template <int T, int R, int WARPS, int NS, int MINB, bool PM = false>
 cudaError_t launch_cfg(const Launch &L, int nctas, cudaStream_t st)
 {
     using Y = Lay<T, R, WARPS, NS>;
@@ -541,7 +567,7 @@ cudaError_t launch_cfg(const Launch &L, int nctas, cudaStream_t st)
     if (!encode_map(&M.m[kMapIn], L.in, L, TILE_Y) || !encode_map(&M.m[kMapOut], L.out, L, TILE_Y) ||
         !encode_map(&M.m[kMapScratch], L.scratch, L, TILE_Y))
         return cudaErrorNotSupported;
-    auto kern = idg_stream_kernel<T, R, WARPS, NS, MINB>;
+    auto kern = idg_stream_kernel<T, R, WARPS, NS, MINB, PM>;
     static bool attr_done = false;
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Y::kBytes);
@@ -567,6 +593,15 @@ bool stream_supported(int nx, int ny, int nz, const void *in, const void *out, c
 //       | 3 = 128x40 tile, 320 threads, two CTAs per SM | 4 = 128x80 tile, 640 threads, one CTA per SM
 cudaError_t launch_stream(const Launch &L, int nctas, int tile, cudaStream_t st)
 {
+    if (L.mode == 1) {          // gradient-driven variant: the two standard tilings, T <= 2
+        switch (L.fuse * 10 + tile) {
+        case 10: case 11: return launch_cfg<1, 4, 16, 5, 1, true>(L, nctas, st);
+        case 12: return launch_cfg<1, 4, 8, 5, 2, true>(L, nctas, st);
+        case 20: case 21: return launch_cfg<2, 4, 16, 5, 1, true>(L, nctas, st);
+        case 22: return launch_cfg<2, 4, 8, 5, 2, true>(L, nctas, st);
+        default: return cudaErrorInvalidValue;
+        }
+    }
     switch (L.fuse * 10 + tile) {
     case 10: case 11: return launch_cfg<1, 4, 16, 5, 1>(L, nctas, st);
     case 12: return launch_cfg<1, 4, 8, 5, 2>(L, nctas, st);
