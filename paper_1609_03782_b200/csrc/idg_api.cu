@@ -98,7 +98,12 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
         // kernel (one tile column, no idle tail between cubes); large single cubes on the z-chunked TMA
         // kernel with two CTAs per SM; cubes too small to fill the GPU want few, deeply fused launches.
         const double work = (double)N * (double)batch;
-        if (can_stream && (batch > 1 || nx <= 128) && work >= 4.0e6) {
+        // the persistent kernel pays ~2T + 3 warm-up planes per CTA: it wants >= 24 planes per team
+        // (two 128x32-tile CTAs per SM; x tiles of 30 float4 + one halo column each)
+        const int nx4 = nx / 4, tiles_x = nx4 <= 2 ? 1 : (nx4 - 2 + 29) / 30, tiles_y = (ny + 27) / 28;
+        const double teams = (double)(296 / (tiles_x < 296 ? tiles_x : 296));
+        const double planes_per_team = (double)batch * tiles_y * (double)nz / (teams < 1.0 ? 1.0 : teams);
+        if (can_stream && (batch > 1 || nx <= 128) && planes_per_team >= 24.0) {
             kernel = 4;
             if (!fuse) fuse = 2;
             if (!tile) tile = 2;
