@@ -9,7 +9,8 @@
 // while the current one is filtered), an x pass (4 consecutive outputs per item from aligned float4
 // loads) and a y pass (4 rows per thread from a register window) give the xy-filtered plane, which
 // enters a ring of 2 rz + 1 planes; the z pass combines the ring into one output plane.  Ring entries
-// are private to the thread that wrote them, so a plane step needs two CTA barriers.  The cube is read
+// are private to the thread that wrote them (a register shift array for rz <= 4, shared memory
+// above), so a plane step needs two CTA barriers.  The cube is read
 // once and written once (8 B per voxel plus halo), instead of three round trips for three 1-D passes.
 //
 // The radii are template parameters (everything unrolls, no address arithmetic is left in the plane
@@ -42,8 +43,11 @@ struct Geo {
     static constexpr int NV = (OFF + 4 + 2 * RXY + 3) / 4;   // float4 loads per x-pass item
     static constexpr int W = 2 * RZ + 1;
     static constexpr int ROW_IT = ROWS_PAD / 8, COL_IT = (COLS + 31) / 32;
-    static constexpr size_t kSmem = sizeof(float) * ((size_t)ROWS_PAD * STRIDE + (size_t)ROWS * TX + (size_t)W * TY * TX);
-    static constexpr int kMinBlocks = kSmem * 3 <= 200 * 1024 ? 3 : (kSmem * 2 <= 220 * 1024 ? 2 : 1);
+    static constexpr bool REG_RING = RZ <= 4;                // z ring in registers (4 W per thread) or in shared memory
+    static constexpr size_t kSmem = sizeof(float) * ((size_t)ROWS_PAD * STRIDE + (size_t)ROWS * TX +
+                                                     (REG_RING ? 0 : (size_t)W * TY * TX));
+    // register budget: the z shift array costs 4 W registers per thread
+    static constexpr int kMinBlocks = REG_RING ? (RZ <= 2 ? 3 : 2) : (kSmem * 3 <= 200 * 1024 ? 3 : (kSmem * 2 <= 220 * 1024 ? 2 : 1));
 };
 
 template <int RXY, int RZ>
@@ -93,6 +97,11 @@ __global__ void __launch_bounds__(NT, Geo<RXY, RZ>::kMinBlocks) idg_sep3d_kernel
     fetch(q_first);
     int slot = 0;
     float *ring_col = ring + (4 * yg) * TX + xl;
+    float zr[G::REG_RING ? G::W : 1][4];
+#pragma unroll
+    for (int k = 0; k < (G::REG_RING ? G::W : 1); ++k)
+#pragma unroll
+        for (int o = 0; o < 4; ++o) zr[k][o] = 0.f;
     const bool col_ok = x0 + xl < S.nx;
     for (int q = q_first; q <= q_last; ++q) {
         stash();
@@ -131,20 +140,38 @@ __global__ void __launch_bounds__(NT, Geo<RXY, RZ>::kMinBlocks) idg_sep3d_kernel
 #pragma unroll
                 for (int o = 0; o < 4; ++o) p[o] = fmaf(S.wy[k], win[o + k], p[o]);
         }
-        // my four ring entries of the slot of plane q (private to this thread)
-#pragma unroll
-        for (int o = 0; o < 4; ++o) ring_col[(slot * TY + o) * TX] = p[o];
         const int zo = q - RZ;                        // output plane whose window [zo-rz, zo+rz] is now complete
-        slot = (slot + 1 == G::W) ? 0 : slot + 1;     // slot of plane q - 2 RZ = zo - RZ (and of plane q + 1)
-        if (zo >= z0) {
-            float acc[4] = {0.f, 0.f, 0.f, 0.f};
-            int sl = slot;
+        float acc[4] = {0.f, 0.f, 0.f, 0.f};
+        if (G::REG_RING) {
+            // shift register of my last W xy-filtered values: zr[k] = plane zo - RZ + k
 #pragma unroll
-            for (int k = 0; k < G::W; ++k) {
+            for (int k = 0; k + 1 < G::W; ++k)
 #pragma unroll
-                for (int o = 0; o < 4; ++o) acc[o] = fmaf(S.wz[k], ring_col[(sl * TY + o) * TX], acc[o]);
-                sl = (sl + 1 == G::W) ? 0 : sl + 1;
+                for (int o = 0; o < 4; ++o) zr[k][o] = zr[k + 1][o];
+#pragma unroll
+            for (int o = 0; o < 4; ++o) zr[G::W - 1][o] = p[o];
+            if (zo >= z0) {
+#pragma unroll
+                for (int k = 0; k < G::W; ++k)
+#pragma unroll
+                    for (int o = 0; o < 4; ++o) acc[o] = fmaf(S.wz[k], zr[k][o], acc[o]);
             }
+        } else {
+            // my four ring entries of the slot of plane q (private to this thread)
+#pragma unroll
+            for (int o = 0; o < 4; ++o) ring_col[(slot * TY + o) * TX] = p[o];
+            slot = (slot + 1 == G::W) ? 0 : slot + 1; // slot of plane q - 2 RZ = zo - RZ (and of plane q + 1)
+            if (zo >= z0) {
+                int sl = slot;
+#pragma unroll
+                for (int k = 0; k < G::W; ++k) {
+#pragma unroll
+                    for (int o = 0; o < 4; ++o) acc[o] = fmaf(S.wz[k], ring_col[(sl * TY + o) * TX], acc[o]);
+                    sl = (sl + 1 == G::W) ? 0 : sl + 1;
+                }
+            }
+        }
+        if (zo >= z0) {
             if (col_ok) {
                 float *dst = S.out + (size_t)zo * plane + (size_t)(y0 + 4 * yg) * S.nx + x0 + xl;
 #pragma unroll
