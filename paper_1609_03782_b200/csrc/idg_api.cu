@@ -12,7 +12,7 @@
 
 namespace {
 
-int g_opt[IDG_OPT_COUNT_] = {0, 0, 0, 0, 0};
+int g_opt[IDG_OPT_COUNT_] = {0, 0, 0, 0, 0, 0};
 thread_local int t_launches = 0;
 thread_local char t_plan[96] = "none";
 
@@ -306,10 +306,85 @@ int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
     float *d_in = (float *)base, *d_out = (float *)(base + cube_al);
     void *ws = base + 2 * cube_al;
     int rc = IDG_OK;
-    e = cudaMemcpyAsync(d_in, cube_host, bytes, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) {
-        rc = run(d_in, nx, ny, nz, 1, nullptr, n_iter, params, d_out, ws, ws_bytes, st);
-        if (rc == IDG_OK) e = cudaMemcpyAsync(out_host, d_out, bytes, cudaMemcpyDeviceToHost, st);
+    e = cudaSuccess;
+
+    // Slab pipeline: the paper's T_p includes the transfers, and on a PCIe link they
+    // dominate.  The cube is cut into z slabs; slab s is filtered on planes [z0-n, z1+n) (an error made
+    // at an artificial slab face travels one plane per iteration, so after n iterations planes [z0, z1)
+    // are exact: domain of dependence, pinned by P8) while slab s+1 is still arriving and slab s-1 is
+    // leaving, on two internal copy streams.  Results are bit-identical to the one-piece path.
+    int slabs = g_opt[IDG_OPT_HOST_SLABS];
+    if (slabs == 0) {
+        slabs = 1;
+        if (bytes >= (64u << 20) && n_iter > 0) {
+            const int thick = 4 * n_iter > 16 ? 4 * n_iter : 16;       // keep the halo overhead below ~50 %
+            slabs = nz / thick;
+            if (slabs > 8) slabs = 8;
+            if (slabs < 1) slabs = 1;
+        }
+    }
+    if (slabs > nz) slabs = nz;
+    const size_t plane_b = (size_t)nx * ny * sizeof(float);
+    const int zs = (nz + slabs - 1) / slabs;
+    const int max_planes = zs + 2 * n_iter < nz ? zs + 2 * n_iter : nz;
+    const size_t slab_al = align_up((size_t)max_planes * plane_b);
+    const size_t slab_ws = idg_workspace_bytes(nx, ny, max_planes, 1);
+    if (slabs > 1 && n_iter > 0 && 2 * slab_al + slab_ws <= need - cube_al) {
+        static cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+        static cudaEvent_t ev_h[8], ev_c[8], ev_d[8], ev_begin;
+        static bool ready = false;
+        if (!ready) {
+            e = cudaStreamCreateWithFlags(&s_h2d, cudaStreamNonBlocking);
+            if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s_d2h, cudaStreamNonBlocking);
+            for (int i = 0; i < 8 && e == cudaSuccess; ++i) {
+                e = cudaEventCreateWithFlags(&ev_h[i], cudaEventDisableTiming);
+                if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_c[i], cudaEventDisableTiming);
+                if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_d[i], cudaEventDisableTiming);
+            }
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_begin, cudaEventDisableTiming);
+            ready = (e == cudaSuccess);
+        }
+        char *region = base + cube_al;
+        float *d_slab[2] = {(float *)region, (float *)(region + slab_al)};
+        void *ws_slab = region + 2 * slab_al;
+        int launches = 0, copied = 0;                                   // planes of I_0 already requested
+        if (e == cudaSuccess) e = cudaEventRecord(ev_begin, st);         // earlier work on `st` may own the buffers
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s_h2d, ev_begin, 0);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s_d2h, ev_begin, 0);
+        for (int sl = 0; sl < slabs && e == cudaSuccess && rc == IDG_OK; ++sl) {
+            const int z0 = sl * zs, z1 = z0 + zs < nz ? z0 + zs : nz;
+            if (z0 >= z1) break;
+            const int lo = z0 - n_iter > 0 ? z0 - n_iter : 0, hi = z1 + n_iter < nz ? z1 + n_iter : nz;
+            if (hi > copied) {
+                e = cudaMemcpyAsync((char *)d_in + (size_t)copied * plane_b, (const char *)cube_host + (size_t)copied * plane_b,
+                                    (size_t)(hi - copied) * plane_b, cudaMemcpyHostToDevice, s_h2d);
+                copied = hi;
+            }
+            if (e == cudaSuccess) e = cudaEventRecord(ev_h[sl], s_h2d);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_h[sl], 0);
+            if (e == cudaSuccess && sl >= 2) e = cudaStreamWaitEvent(st, ev_d[sl - 2], 0);     // its output buffer is free
+            if (e != cudaSuccess) break;
+            float *d_o = d_slab[sl & 1];
+            rc = run(d_in + (size_t)lo * nx * ny, nx, ny, hi - lo, 1, nullptr, n_iter, params, d_o, ws_slab, slab_ws, st);
+            launches += t_launches;
+            if (rc != IDG_OK) break;
+            e = cudaEventRecord(ev_c[sl], st);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(s_d2h, ev_c[sl], 0);
+            if (e == cudaSuccess)
+                e = cudaMemcpyAsync((char *)out_host + (size_t)z0 * plane_b, (const char *)d_o + (size_t)(z0 - lo) * plane_b,
+                                    (size_t)(z1 - z0) * plane_b, cudaMemcpyDeviceToHost, s_d2h);
+            if (e == cudaSuccess) e = cudaEventRecord(ev_d[sl], s_d2h);
+            if (e == cudaSuccess && sl == slabs - 1) e = cudaStreamWaitEvent(st, ev_d[sl], 0);  // `st` ends after the last copy
+        }
+        t_launches = launches;
+        cudaStreamSynchronize(s_h2d);          // on an error path the copies must not outlive the buffers
+        cudaStreamSynchronize(s_d2h);
+    } else {
+        e = cudaMemcpyAsync(d_in, cube_host, bytes, cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) {
+            rc = run(d_in, nx, ny, nz, 1, nullptr, n_iter, params, d_out, ws, ws_bytes, st);
+            if (rc == IDG_OK) e = cudaMemcpyAsync(out_host, d_out, bytes, cudaMemcpyDeviceToHost, st);
+        }
     }
     if (own) {
         cudaError_t e2 = cudaFreeAsync(base, st);
@@ -523,6 +598,7 @@ int idg_set_option(int key, int value)
     if (key == IDG_OPT_ZCHUNK && value < 0) return IDG_ERR_OPTION;
     if (key == IDG_OPT_TILE && (value < 0 || value > 4)) return IDG_ERR_OPTION;
     if (key == IDG_OPT_CTAS && value < 0) return IDG_ERR_OPTION;
+    if (key == IDG_OPT_HOST_SLABS && (value < 0 || value > 8)) return IDG_ERR_OPTION;
     g_opt[key] = value;
     return IDG_OK;
 }

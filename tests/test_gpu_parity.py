@@ -323,6 +323,30 @@ def test_host_entry_point(B, oracle):
     assert torch.equal(out, out2)
 
 
+@pytest.mark.parametrize("slabs", [2, 3, 8])
+def test_host_entry_point_slab_pipeline(B, oracle, slabs):
+    """idg_filter_host cut into z slabs (upload / filter / download overlapped): every slab is filtered with
+    n halo planes per side, so the result is bit-identical to the one-piece call (domain of dependence, P8);
+    slabs thinner than the halo, a ragged last slab and device buffers supplied by the caller."""
+    set_plan(B, (0, 0))
+    rng = np.random.default_rng(31)
+    a = (rng.normal(0, 1, (45, 40, 64)) + 8.0 * (rng.random((45, 40, 64)) < 0.05)).astype(np.float32)
+    p = B.Params(K=1.5, tau=0.03, cx=5.0, cy=4.0, cz=6.0, rms=1.0)
+    h = torch.from_numpy(a).pin_memory()
+    dev = torch.empty(B.host_buffers_bytes(64, 40, 45), dtype=torch.uint8, device="cuda")
+    for n in (1, 4, 9):
+        B.idg_set_option(B.IDG_OPT_HOST_SLABS, 1)
+        one = B.idg_filter_host(h, n, p, dev_buffers=dev).clone()
+        B.idg_set_option(B.IDG_OPT_HOST_SLABS, slabs)
+        try:
+            out = B.idg_filter_host(h, n, p, dev_buffers=dev)
+            out_own = B.idg_filter_host(h, n, p)
+        finally:
+            B.idg_set_option(B.IDG_OPT_HOST_SLABS, 0)
+        assert torch.equal(out, one) and torch.equal(out_own, one), (slabs, n)
+        assert err(out.numpy(), oracle.idg_filter_oracle(a, n, **p.f32()), 1.0) <= TOL
+
+
 def test_argument_errors(B):
     from paper_1609_03782_b200.binding import IdgError
     t = torch.zeros(4, 4, 4, device="cuda")
