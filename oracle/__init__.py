@@ -20,7 +20,8 @@ from typing import Optional
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SRC = [os.path.join(_HERE, "idg_oracle.c"), os.path.join(_HERE, "ref_filters_oracle.c")]
+_SRC = [os.path.join(_HERE, "idg_oracle.c"), os.path.join(_HERE, "ref_filters_oracle.c"),
+        os.path.join(_HERE, "wavelet_oracle.c")]
 _LIB = os.path.join(_HERE, "libidg_oracle.so")
 _lib: Optional[ctypes.CDLL] = None
 
@@ -48,6 +49,13 @@ def _load() -> ctypes.CDLL:
                                        ctypes.c_double, ctypes.c_double, ctypes.c_double, dp, dp]
         lib.idg_oracle_set_threads.restype = ctypes.c_int
         lib.idg_oracle_set_threads.argtypes = [ctypes.c_int]
+        i_ = ctypes.c_int
+        lib.wavelet_forward_oracle.restype = i_
+        lib.wavelet_forward_oracle.argtypes = [dp, i_, i_, i_, i_, i_]
+        lib.wavelet_inverse_oracle.restype = i_
+        lib.wavelet_inverse_oracle.argtypes = [dp, i_, i_, i_, i_, i_]
+        lib.wavelet_filter_oracle.restype = i_
+        lib.wavelet_filter_oracle.argtypes = [dp, i_, i_, i_, i_, i_, dp, ctypes.c_double, dp]
         lib.pm_oracle_f64.restype = ctypes.c_int
         lib.pm_oracle_f64.argtypes = lib.idg_oracle_f64.argtypes
         ip = ctypes.POINTER(ctypes.c_int)
@@ -167,4 +175,36 @@ def gaussian_filter_oracle(cube: np.ndarray, fwhm, theta=(0.0, 0.0, 0.0)) -> np.
                                      out.ctypes.data_as(dp))
     if rc != 0:
         raise ValueError(f"gaussian_oracle_f64 rejected its arguments (rc={rc})")
+    return out
+
+
+HAAR, LEGALL = 0, 1
+
+
+def wavelet_transform_oracle(cube: np.ndarray, wavelet: int, levels: int, inverse: bool = False) -> np.ndarray:
+    """Forward (or inverse) lifting transform to `levels` (Eq. 8-11), coefficients
+    interleaved in place: c at even, d at odd lattice positions.  wavelet: HAAR or LEGALL."""
+    a = np.array(cube, dtype=np.float64, order="C", copy=True)
+    if a.ndim != 3:
+        raise ValueError("cube must be 3-D [nz, ny, nx]")
+    nz, ny, nx = a.shape
+    dp = ctypes.POINTER(ctypes.c_double)
+    fn = _load().wavelet_inverse_oracle if inverse else _load().wavelet_forward_oracle
+    if fn(a.ctypes.data_as(dp), nx, ny, nz, int(wavelet), int(levels)) != 0:
+        raise ValueError("wavelet oracle rejected its arguments")
+    return a
+
+
+def wavelet_filter_oracle(cube: np.ndarray, wavelet: int, thresholds, rms: float = 1.0) -> np.ndarray:
+    """Wavelet thresholding filter: decompose to len(thresholds) levels, zero every
+    coefficient with |v| < t_l * rms (detail bands of level l, approximation band with t_L), transform back."""
+    a = _cube64(cube)
+    nz, ny, nx = a.shape
+    out = np.empty_like(a)
+    t = np.ascontiguousarray(thresholds, dtype=np.float64)
+    dp = ctypes.POINTER(ctypes.c_double)
+    rc = _load().wavelet_filter_oracle(a.ctypes.data_as(dp), nx, ny, nz, int(wavelet), int(t.size),
+                                       t.ctypes.data_as(dp), float(rms), out.ctypes.data_as(dp))
+    if rc != 0:
+        raise ValueError(f"wavelet_filter_oracle rejected its arguments (rc={rc})")
     return out
