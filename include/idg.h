@@ -213,6 +213,35 @@ int idg_quality(const double *sums, double rms_o, double rms_f, double voxels_pe
                 double *F_M);
 
 /*
+ * Wavelet lifting (section 3.4).  One level along a line: split into even and odd
+ * samples, predict d_i = odd_i - P(even) (Eq. 8), update c_i = even_i + U(d) (Eq. 10), with
+ *   Haar          P = even_i (Eq. 9),               U = d_i / 2 (Eq. 11)
+ *   Le Gall 5/3   P = (even_i + even_{i+1}) / 2,    U = (d_{i-1} + d_i) / 4   (symmetric extension at the ends)
+ * Coefficients stay interleaved in place: after level l the approximation band lives on
+ * the voxels whose three indices are multiples of 2^l.  Per level the lines along x, then y, then z of
+ * the current lattice are transformed (readings W1-W5).
+ */
+enum { IDG_WAVELET_HAAR = 0, IDG_WAVELET_LEGALL53 = 1 };
+
+/*
+ * Forward (inverse = 0) or inverse (inverse != 0) transform to `levels` (0..16) of a cube.
+ *   cube [device] nx*ny*nz fp32;  out [device] nx*ny*nz fp32, may equal cube (in place), else disjoint
+ */
+int idg_wavelet_transform(const float *cube, int nx, int ny, int nz, int wavelet, int levels, int inverse, float *out,
+                          void *stream);
+
+/*
+ * Wavelet thresholding filter: transform to `levels` (1..16; the paper stops at 3), set to
+ * zero every coefficient with |v| < t_l * rms -- detail coefficients created at level l with t_l, the
+ * approximation band with t_levels ("it is necessary to threshold both the detail and approximation
+ * bands") -- and transform back.  Pre-smoothing is a separate idg_gaussian_filter call.
+ *   thresholds [host] `levels` floats >= 0, in units of rms;  rms > 0: noise level of the original cube
+ *   cube, out as for idg_wavelet_transform.  Invalid wavelet, levels, thresholds or rms: IDG_ERR_PARAM.
+ */
+int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, int levels, const float *thresholds,
+                       float rms, float *out, void *stream);
+
+/*
  * Process-wide tuning knobs (tests and benchmarks; defaults give the fastest plan).
  *   IDG_OPT_KERNEL   0 auto | 1 naive (one thread per voxel) | 2 tiled z-streaming kernel (global loads)
  *                    | 3 tiled z-streaming kernel fed by TMA | 4 persistent warp-decoupled TMA kernel

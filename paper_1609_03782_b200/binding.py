@@ -25,7 +25,9 @@ SYMBOLS = ("idg_version", "idg_status_string", "idg_params_check", "idg_workspac
            "idg_filter", "idg_filter_ws", "idg_filter_batched", "idg_filter_host",
            "idg_set_option", "idg_get_option", "idg_last_launch_count", "idg_last_plan",
            "idg_box_filter", "idg_gaussian_filter", "idg_gaussian_radii",
-           "idg_mask_sums", "idg_cube_stats", "idg_quality", "idg_filter_pm")
+           "idg_mask_sums", "idg_cube_stats", "idg_quality", "idg_filter_pm",
+           "idg_wavelet_transform", "idg_wavelet_filter")
+WAVELET_HAAR, WAVELET_LEGALL53 = 0, 1
 
 
 class IdgParams(ctypes.Structure):
@@ -113,6 +115,10 @@ def lib() -> ctypes.CDLL:
         L.idg_cube_stats.argtypes = [fp, i, i, i, rp, vp, vp]
         L.idg_quality.restype = i
         L.idg_quality.argtypes = [dptr, d, d, d, dptr, dptr, dptr]
+        L.idg_wavelet_transform.restype = i
+        L.idg_wavelet_transform.argtypes = [fp, i, i, i, i, i, i, fp, vp]
+        L.idg_wavelet_filter.restype = i
+        L.idg_wavelet_filter.argtypes = [fp, i, i, i, i, i, ctypes.POINTER(ctypes.c_float), f, fp, vp]
         _lib = L
     return _lib
 
@@ -335,6 +341,31 @@ def idg_quality(sums: Sequence[float], rms_o: float, rms_f: float, voxels_per_be
     _check(lib().idg_quality(arr, float(rms_o), float(rms_f), float(voxels_per_beam),
                              *[ctypes.byref(o) for o in out]))
     return {"F": out[0].value, "sigma_F": out[1].value, "F_M": out[2].value}
+
+
+def idg_wavelet_transform(cube: torch.Tensor, wavelet: int, levels: int, inverse: bool = False,
+                          out: Optional[torch.Tensor] = None,
+                          stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """idg_wavelet_transform on a [nz, ny, nx] CUDA tensor (out may be the cube itself: in place)."""
+    nz, ny, nx = cube.shape
+    if out is None:
+        out = torch.empty_like(cube)
+    _check(lib().idg_wavelet_transform(_dev(cube, "cube"), nx, ny, nz, int(wavelet), int(levels), int(bool(inverse)),
+                                       _dev(out, "out"), _stream(stream)))
+    return out
+
+
+def idg_wavelet_filter(cube: torch.Tensor, wavelet: int, thresholds: Sequence[float], rms: float = 1.0,
+                       out: Optional[torch.Tensor] = None,
+                       stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """idg_wavelet_filter: len(thresholds) levels, thresholds in units of rms."""
+    nz, ny, nx = cube.shape
+    if out is None:
+        out = torch.empty_like(cube)
+    t = (ctypes.c_float * max(1, len(thresholds)))(*[float(v) for v in thresholds])
+    _check(lib().idg_wavelet_filter(_dev(cube, "cube"), nx, ny, nz, int(wavelet), len(thresholds), t, float(rms),
+                                    _dev(out, "out"), _stream(stream)))
+    return out
 
 
 def host_buffers_bytes(nx: int, ny: int, nz: int) -> int:

@@ -590,6 +590,64 @@ int idg_quality(const double *sums, double rms_o, double rms_f, double voxels_pe
     return IDG_OK;
 }
 
+// ---- wavelet lifting (section 3.4, Eq. 8-11) ------------------------------------------
+
+static int wavelet_args(const float *cube, int nx, int ny, int nz, int wavelet, int levels, const float *out, size_t *N)
+{
+    if (!cube || !out) return IDG_ERR_NULL;
+    if (!voxel_count(nx, ny, nz, 1, N)) return IDG_ERR_DIMS;
+    if ((wavelet != IDG_WAVELET_HAAR && wavelet != IDG_WAVELET_LEGALL53) || levels < 0 || levels > 16) return IDG_ERR_PARAM;
+    if ((const float *)out != cube && ranges_overlap(cube, *N * sizeof(float), out, *N * sizeof(float)))
+        return IDG_ERR_OVERLAP;
+    return IDG_OK;
+}
+
+int idg_wavelet_transform(const float *cube, int nx, int ny, int nz, int wavelet, int levels, int inverse, float *out,
+                          void *stream)
+{
+    t_launches = 0;
+    size_t N;
+    const int rc = wavelet_args(cube, nx, ny, nz, wavelet, levels, out, &N);
+    if (rc != IDG_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaSuccess;
+    if ((const float *)out != cube) e = cudaMemcpyAsync(out, cube, N * sizeof(float), cudaMemcpyDeviceToDevice, st);
+    int launches = 0;
+    if (e == cudaSuccess) e = idg::launch_wavelet_transform(out, nx, ny, nz, wavelet, levels, inverse != 0, st, &launches);
+    if (e != cudaSuccess) return (int)e;
+    t_launches = launches;
+    snprintf(t_plan, sizeof(t_plan), "idg_lift_kernel %s levels=%d %s", wavelet == 0 ? "haar" : "legall53", levels,
+             inverse ? "inverse" : "forward");
+    return IDG_OK;
+}
+
+int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, int levels, const float *thresholds,
+                       float rms, float *out, void *stream)
+{
+    t_launches = 0;
+    size_t N;
+    const int rc = wavelet_args(cube, nx, ny, nz, wavelet, levels, out, &N);
+    if (rc != IDG_OK) return rc;
+    if (!thresholds) return IDG_ERR_NULL;
+    if (levels < 1 || !(rms > 0.0f) || !isfinite(rms)) return IDG_ERR_PARAM;
+    float thr[16];
+    for (int l = 0; l < levels; ++l) {
+        if (!(thresholds[l] >= 0.0f)) return IDG_ERR_PARAM;                 // also rejects NaN
+        thr[l] = (float)((double)thresholds[l] * (double)rms);              // t_l in units of rms
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaSuccess;
+    if ((const float *)out != cube) e = cudaMemcpyAsync(out, cube, N * sizeof(float), cudaMemcpyDeviceToDevice, st);
+    int launches = 0;
+    if (e == cudaSuccess) e = idg::launch_wavelet_transform(out, nx, ny, nz, wavelet, levels, false, st, &launches);
+    if (e == cudaSuccess) { e = idg::launch_wavelet_threshold(out, nx, ny, nz, levels, thr, st); ++launches; }
+    if (e == cudaSuccess) e = idg::launch_wavelet_transform(out, nx, ny, nz, wavelet, levels, true, st, &launches);
+    if (e != cudaSuccess) return (int)e;
+    t_launches = launches;
+    snprintf(t_plan, sizeof(t_plan), "idg_lift_kernel %s levels=%d filter", wavelet == 0 ? "haar" : "legall53", levels);
+    return IDG_OK;
+}
+
 int idg_set_option(int key, int value)
 {
     if (key < 0 || key >= IDG_OPT_COUNT_) return IDG_ERR_OPTION;

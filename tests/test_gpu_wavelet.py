@@ -1,0 +1,105 @@
+"""GPU parity of the wavelet lifting path (section 3.4, Eq. 8-11): idg_wavelet_transform and
+idg_wavelet_filter through the C ABI against oracle/wavelet_oracle.c.
+
+Transform coefficients are compared element by element (fp32 lifting against fp64: 1e-4 x rms, in
+practice ~1e-6).  The filter takes a hard decision per coefficient; where the fp64 coefficient lies
+within MARGIN of its threshold either decision is correct, so the test compares what is unique (all
+other coefficients must follow the oracle's decision) and checks that the ambiguous ones are either
+kept or cut."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+MARGIN = 1e-4
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1609_03782_b200 import binding
+    binding.lib()
+    return binding
+
+
+def noisy(shape, seed):
+    rng = np.random.default_rng(seed)
+    return (rng.normal(0, 1, shape) + 8.0 * (rng.random(shape) < 0.03)).astype(np.float32)
+
+
+SHAPES = [(1, 1, 1), (1, 1, 2), (1, 1, 5), (4, 4, 4), (5, 6, 7), (3, 1, 9), (9, 10, 17), (21, 67, 100), (16, 64, 128),
+          (33, 40, 130)]
+IDS = lambda s: "x".join(map(str, s[::-1])) if isinstance(s, tuple) else None
+
+
+def level_map(shape, levels):
+    idx = np.indices(shape)
+    tz = lambda p: np.where(p == 0, 31, np.log2(np.maximum(p & -p, 1)).astype(int))
+    return np.minimum(np.minimum(np.minimum(tz(idx[0]), tz(idx[1])), tz(idx[2])) + 1, levels)
+
+
+@pytest.mark.parametrize("wavelet", [0, 1], ids=["haar", "legall"])
+@pytest.mark.parametrize("shape", SHAPES, ids=IDS)
+def test_transform_and_inverse(B, oracle, shape, wavelet):
+    a = noisy(shape, 21)
+    t = torch.from_numpy(a).cuda()
+    for L in (0, 1, 2, 3, 5):
+        w = B.idg_wavelet_transform(t, wavelet, L)
+        ref = oracle.wavelet_transform_oracle(a, wavelet, L)
+        assert np.abs(w.cpu().numpy().astype(np.float64) - ref).max() <= TOL, (shape, L)
+        back = B.idg_wavelet_transform(w, wavelet, L, inverse=True)
+        assert float((back - t).abs().max()) <= TOL                      # reversible
+        inplace = t.clone()
+        B.idg_wavelet_transform(inplace, wavelet, L, out=inplace)
+        assert torch.equal(inplace, w)                                   # in place == out of place
+
+
+@pytest.mark.parametrize("wavelet,thr", [(0, (0.5, 0.8, 1.1)), (1, (1.0, 1.4, 1.7)), (0, (0.7,)), (1, (0.6, 1.15))],
+                         ids=["haar-paper", "legall-paper", "haar-l1", "legall-l2"])
+@pytest.mark.parametrize("shape", [(5, 6, 7), (9, 10, 17), (21, 67, 100), (33, 40, 130)], ids=IDS)
+def test_filter(B, oracle, shape, wavelet, thr):
+    """Thresholds of PAPER.md:222 (Haar 0.5/0.8/1.1, Le Gall 1/1.4/1.7 x rms) and two of the sweep."""
+    rms = 1.5
+    a = (noisy(shape, 22) * rms).astype(np.float32)
+    L = len(thr)
+    out = B.idg_wavelet_filter(torch.from_numpy(a).cuda(), wavelet, thr, rms).cpu().numpy().astype(np.float64)
+    w = oracle.wavelet_transform_oracle(a, wavelet, L)                   # fp64 coefficients
+    t_map = np.asarray([float(np.float32(t)) * rms for t in thr])[level_map(shape, L) - 1]
+    ambiguous = np.abs(np.abs(w) - t_map) <= MARGIN * rms
+    got = oracle.wavelet_transform_oracle(out, wavelet, L)               # coefficients the GPU kept
+    want = np.where(np.abs(w) < t_map, 0.0, w)
+    assert np.abs(got - want)[~ambiguous].max() <= TOL * rms             # what is unique
+    amb = got[ambiguous]
+    ok = np.minimum(np.abs(amb), np.abs(amb - w[ambiguous])) <= TOL * rms
+    assert ok.all()                                                      # the rest: kept or cut
+    if not ambiguous.any():
+        assert np.abs(out - oracle.wavelet_filter_oracle(a, wavelet, [float(np.float32(t)) for t in thr], rms)).max() <= TOL * rms
+
+
+def test_filter_limits_and_config0(B, oracle):
+    from paper_1609_03782_b200 import synth
+    c = synth.modelb_like(seed=1000, snr=32.0)
+    t = torch.from_numpy(c.data).cuda()
+    for wv in (0, 1):
+        assert float((B.idg_wavelet_filter(t, wv, (0.0, 0.0, 0.0)) - t).abs().max()) <= TOL      # t = 0: identity
+        assert float(B.idg_wavelet_filter(t, wv, (1e9,)).abs().max()) == 0.0                      # everything cut
+    # the paper's recipe: Gaussian pre-smoothing, then the wavelet filter (FWHM 3 for the models)
+    pre = B.idg_gaussian_filter(t, (3, 3, 3))
+    out = B.idg_wavelet_filter(pre, B.WAVELET_HAAR, (0.5, 0.8, 1.1), c.rms)
+    assert float((out == 0).float().mean()) > 0.3 and float(out.max()) > 10.0     # noise cut, bright disc kept
+
+
+def test_argument_errors(B):
+    a = torch.zeros((4, 5, 8), device="cuda")
+    for args in ((2, (0.5,), 1.0), (0, (), 1.0), (0, (-1.0,), 1.0), (0, (0.5,), 0.0), (1, (float("nan"),), 1.0)):
+        with pytest.raises(B.IdgError) as e:
+            B.idg_wavelet_filter(a, *args)
+        assert e.value.status == -4
+    with pytest.raises(B.IdgError) as e:
+        B.idg_wavelet_transform(a, 0, 17)
+    assert e.value.status == -4
+    with pytest.raises(TypeError):
+        B.idg_wavelet_transform(a.cpu(), 0, 1)
