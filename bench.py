@@ -43,7 +43,8 @@ BATCH = 256
 FILTERS = {"idg": None, "box": ("box", (3, 3, 3)), "box_aniso": ("box", (3, 5, 5)),
            "gauss": ("gauss", (3.0, 3.0, 3.0), (0.0, 0.0, 0.0)), "gauss_aniso": ("gauss", (2.0, 3.0, 3.0), (0.0, 0.0, 0.0)),
            "gauss_rot": ("gauss", (2.0, 3.0, 3.0), (10.0, 20.0, 30.0)),
-           "mask_sums": ("quality",)}                 # Eq. 13-14 over the whole cube: reads 2 cubes
+           "mask_sums": ("quality",),
+           "wavelet_haar": ("wavelet", 0, (0.5, 0.8, 1.1)), "wavelet_legall": ("wavelet", 1, (1.0, 1.4, 1.7))}   # PAPER.md:222                 # Eq. 13-14 over the whole cube: reads 2 cubes
 DEFAULT_WORKLOAD = "cfg3_1024x1024x512_n20"
 
 
@@ -261,6 +262,8 @@ def run_ours(args) -> None:
         if filt is not None:
             if filt[0] == "quality":
                 B.idg_mask_sums(d_in, d_out, None, 3.0, 1.5, None, sums=q_sums, stream=stream)
+            elif filt[0] == "wavelet":
+                B.idg_wavelet_filter(d_in, filt[1], filt[2], 1.0, out=d_out, stream=stream)
             elif filt[0] == "box":
                 B.idg_box_filter(d_in, *filt[1], out=d_out, stream=stream)
             else:
@@ -315,6 +318,8 @@ def run_ours(args) -> None:
 
     peak, peak_src = measured_peak_gbs()
     ms_launch = ms_step / launches_per_step
+    if filt is not None and filt[0] == "wavelet":      # many small passes: the roofline unit is the whole filter
+        ms_launch, fuse = ms_step, 1
     achieved = BYTES_PER_VOXEL_ITER * N * fuse / (ms_launch * 1e-3) / 1e9     # algorithmic GB/s per launch
     kernel_tag = f"{plan} {args.workload}"
     if filt is not None:                      # reference filter: its own metric, oracle timed on a small block
@@ -327,6 +332,10 @@ def run_ours(args) -> None:
             blk = data
             t0 = time.perf_counter()
             quality_oracle.mask_sums_oracle(blk, blk, None, 3.0, 1.5)
+        elif filt[0] == "wavelet":
+            blk = data[:min(nz, 128)]
+            t0 = time.perf_counter()
+            oracle.wavelet_filter_oracle(blk, filt[1], filt[2], 1.0)
         elif filt[0] == "box":
             oracle.box_filter_oracle(blk, *filt[1])
         else:
@@ -363,7 +372,7 @@ def run_ours(args) -> None:
         "gpu_launches": launches_per_step * args.steps,
         "clocks": clocks,
     }
-    if filt is not None and len(filt) > 2 and any(filt[2]):     # rotated Gaussian: bound by FP32, not by HBM
+    if filt is not None and filt[0] == "gauss" and any(filt[2]):     # rotated Gaussian: bound by FP32, not by HBM
         r = B.idg_gaussian_radii(filt[1], filt[2])[0]
         flops = 2.0 * (2 * r + 1) ** 3 * N
         peak_tf = 148 * 128 * 2 * 1.965e9 / 1e12          # SMs x FP32 lanes x 2 flop x max clock (B200_PROFILING.md)

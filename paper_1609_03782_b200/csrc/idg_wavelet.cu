@@ -69,6 +69,32 @@ __global__ void __launch_bounds__(NT) idg_lift_kernel(const __grid_constant__ WA
     }
 }
 
+// Haar only: predict and update of one (even, odd) pair touch nothing but the pair (Eq. 8-11 with P = even_i,
+// U = d_i / 2), so both phases run in one race-free in-place pass with a thread per pair; same operations in
+// the same order as the two-phase kernel.
+template <bool INV>
+__global__ void __launch_bounds__(NT) idg_haar_pair_kernel(const __grid_constant__ WArgs W)
+{
+    const int m = W.axis == 0 ? W.mx : (W.axis == 1 ? W.my : W.mz);
+    const int no = m / 2;
+    const int ex = W.axis == 0 ? no : W.mx, ey = W.axis == 1 ? no : W.my, ez = W.axis == 2 ? no : W.mz;
+    const long long total = (long long)ex * ey * ez;
+    const size_t sx = (size_t)W.s, sy = (size_t)W.s * W.nx, sz = (size_t)W.s * W.nx * (size_t)W.ny;
+    const size_t st = W.axis == 0 ? sx : (W.axis == 1 ? sy : sz);
+    for (long long t = (long long)blockIdx.x * NT + threadIdx.x; t < total; t += (long long)gridDim.x * NT) {
+        const int cx = (int)(t % ex), cy = (int)((t / ex) % ey), cz = (int)(t / ((long long)ex * ey));
+        const int i = W.axis == 0 ? cx : (W.axis == 1 ? cy : cz);
+        float *line = W.a + (W.axis == 0 ? 0 : (size_t)cx * sx) + (W.axis == 1 ? 0 : (size_t)cy * sy) +
+                      (W.axis == 2 ? 0 : (size_t)cz * sz);
+        float *pe = line + (size_t)(2 * i) * st, *po = pe + st;
+        float e = *pe, o = *po;
+        if (!INV) { o = o - e; e = e + 0.5f * o; }          // d = odd - even;  c = even + d/2
+        else { e = e - 0.5f * o; o = o + e; }               // even = c - d/2;  odd = d + even
+        *pe = e;
+        *po = o;
+    }
+}
+
 struct TArgs {
     float *a;
     int nx, ny, nz, levels;
@@ -114,6 +140,17 @@ cudaError_t transform(float *a, int nx, int ny, int nz, int levels, bool inverse
             W.axis = inverse ? 2 - ai : ai;
             const int m = W.axis == 0 ? W.mx : (W.axis == 1 ? W.my : W.mz);
             if (m < 2) continue;
+            if (WAVELET == 0) {
+                const long long total = (long long)(W.axis == 0 ? m / 2 : W.mx) * (W.axis == 1 ? m / 2 : W.my) *
+                                        (W.axis == 2 ? m / 2 : W.mz);
+                long long grid = (total + NT - 1) / NT;
+                if (grid > 148LL * 32) grid = 148LL * 32;
+                if (inverse) idg_haar_pair_kernel<true><<<(unsigned)grid, NT, 0, st>>>(W);
+                else idg_haar_pair_kernel<false><<<(unsigned)grid, NT, 0, st>>>(W);
+                e = cudaGetLastError();
+                *launches += 1;
+                continue;
+            }
             if (!inverse) {
                 e = launch_phase<WAVELET, 0, false>(W, st);
                 if (e == cudaSuccess) e = launch_phase<WAVELET, 1, false>(W, st);
