@@ -1,6 +1,7 @@
 // Internal declarations shared by the CUDA translation units of libidg_b200.so.
 // Not part of the public boundary (include/idg.h) and not used by oracle/.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -104,6 +105,10 @@ bool tma_supported(int nx, int ny, int nz, const void *in, const void *out, cons
 cudaError_t launch_stream(const Launch &L, int nctas, int tile, cudaStream_t st);
 bool stream_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
 
+
+// Tensor maps for the TMA kernels (idg_tmap.cu): 4-D (x, y, z, cube), box tile_x x tile_y x 1 x 1, zero fill.
+bool tmap_available();
+bool tmap_encode(CUtensorMap *m, const float *base, int nx, int ny, int nz, int batch, int tile_x, int tile_y);
 
 // Reference filters (PAPER.md sections 3.1-3.2): separable single-pass filter (box, axis-aligned
 // Gaussian) and dense 3-D convolution (rotated Gaussian, Eq. 3).

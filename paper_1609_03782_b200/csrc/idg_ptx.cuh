@@ -65,6 +65,18 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
         "DONE_%=:\n\t}" ::"r"(bar), "r"(parity), "r"(0x989680)   // suspend-time hint: sleep, do not spin
         : "memory");
 }
+// As mbar_wait, without the suspend-time hint (plain try_wait loop).
+__device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(bar), "r"(parity)
+        : "memory");
+}
 // acq_rel counter in shared memory (stage release); returns the old value.
 __device__ __forceinline__ uint32_t atom_add_acq_rel(uint32_t addr, uint32_t v)
 {

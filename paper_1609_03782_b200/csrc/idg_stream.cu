@@ -494,38 +494,9 @@ idg_stream_kernel(const __grid_constant__ Launch L, const __grid_constant__ Stre
     }
 }
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
-                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
-                                  CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encode_fn()
-{
-    static EncodeTiledFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
-        void *p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = (EncodeTiledFn)p;
-    }
-    return fn;
-}
-
 bool encode_map(CUtensorMap *m, const float *base, const Launch &L, int tile_y)
 {
-    EncodeTiledFn fn = encode_fn();
-    if (!fn) return false;
-    const cuuint64_t dims[4] = {(cuuint64_t)L.nx, (cuuint64_t)L.ny, (cuuint64_t)L.nz, (cuuint64_t)L.batch};
-    const cuuint64_t strides[3] = {(cuuint64_t)L.nx * 4, (cuuint64_t)L.nx * L.ny * 4,
-                                   (cuuint64_t)L.nx * L.ny * (cuuint64_t)L.nz * 4};
-    const cuuint32_t box[4] = {(cuuint32_t)kTileX, (cuuint32_t)tile_y, 1, 1};
-    const cuuint32_t estr[4] = {1, 1, 1, 1};
-    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void *)base, dims, strides, box, estr,
-              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    return tmap_encode(m, base, L.nx, L.ny, L.nz, L.batch, kTileX, tile_y);
 }
 
 int sm_count()
@@ -586,7 +557,7 @@ bool stream_supported(int nx, int ny, int nz, const void *in, const void *out, c
     if (nx % 4 != 0 || ny < 4) return false;
     const uintptr_t m = (uintptr_t)in | (uintptr_t)out | (uintptr_t)scratch;
     if ((m & 15u) != 0) return false;
-    return encode_fn() != nullptr;
+    return tmap_available();
 }
 
 // tile: 0 auto | 1 = 128x64 tile, 512 threads, one CTA per SM | 2 = 128x32 tile, 256 threads, two CTAs per SM

@@ -19,6 +19,7 @@
 #include <type_traits>
 
 #include "idg_kernels.cuh"
+#include "idg_ptx.cuh"
 
 namespace idg {
 
@@ -57,12 +58,7 @@ __device__ __forceinline__ Consts make_consts(const CubeParams &p)
     k.one = make_float2(1.0f, 1.0f);
     return k;
 }
-__device__ __forceinline__ float rcp_approx(float x)
-{
-    float r;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
+using ptx::rcp_approx;
 __device__ __forceinline__ float2 update2(float2 c, float2 sx, float2 ym, float2 yp, float2 zm, float2 zp,
                                           const Consts &k)
 {
@@ -96,38 +92,13 @@ __device__ __forceinline__ int mirror(int i, int n)
     return m < n ? m : p - 1 - m;
 }
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p)
+// pointer-taking wrappers over the address-taking helpers of idg_ptx.cuh
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) { ptx::mbar_init(ptx::smem_u32(bar), count); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) { ptx::mbar_expect_tx(ptx::smem_u32(bar), bytes); }
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) { ptx::mbar_wait_spin(ptx::smem_u32(bar), parity); }
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, uint64_t *bar, int x, int y, int z, int b)
 {
-    return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "WAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra DONE_%=;\n\t"
-        "bra WAIT_%=;\n\t"
-        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-}
-// 4-D box load (x, y, z, cube) -> shared memory, completion on `bar`.
-__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, uint64_t *bar, int x, int y,
-                                            int z, int b)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z), "r"(b)
-        : "memory");
+    ptx::tma_load_4d(ptx::smem_u32(dst), map, ptx::smem_u32(bar), x, y, z, b);
 }
 
 struct TmaArgs {
@@ -335,38 +306,9 @@ idg_tma_kernel(const __grid_constant__ Launch L, const __grid_constant__ TmaArgs
     else if (T > 3 && now == 3) tma_body<(T > 3 ? 3 : 1), R, WARPS, NS, T>(map, dst, L, A, prm, b, smem);
 }
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
-                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
-                                  CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encode_fn()
-{
-    static EncodeTiledFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
-        void *p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = (EncodeTiledFn)p;
-    }
-    return fn;
-}
-
 bool encode_map(CUtensorMap *m, const float *base, const Launch &L, int tile_y)
 {
-    EncodeTiledFn fn = encode_fn();
-    if (!fn) return false;
-    const cuuint64_t dims[4] = {(cuuint64_t)L.nx, (cuuint64_t)L.ny, (cuuint64_t)L.nz, (cuuint64_t)L.batch};
-    const cuuint64_t strides[3] = {(cuuint64_t)L.nx * 4, (cuuint64_t)L.nx * L.ny * 4,
-                                   (cuuint64_t)L.nx * L.ny * (cuuint64_t)L.nz * 4};
-    const cuuint32_t box[4] = {(cuuint32_t)kTileX, (cuuint32_t)tile_y, 1, 1};
-    const cuuint32_t estr[4] = {1, 1, 1, 1};
-    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void *)base, dims, strides, box, estr,
-              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    return tmap_encode(m, base, L.nx, L.ny, L.nz, L.batch, kTileX, tile_y);
 }
 
 int pick_zchunk(int nz, long tiles, int T, int slots)
@@ -428,7 +370,7 @@ bool tma_supported(int nx, int ny, int nz, const void *in, const void *out, cons
     if (nx % 4 != 0 || ny < 4) return false;
     const uintptr_t m = (uintptr_t)in | (uintptr_t)out | (uintptr_t)scratch;
     if ((m & 15u) != 0) return false;
-    return encode_fn() != nullptr;
+    return tmap_available();
 }
 
 // tile: 0 auto | 1 = 128x64 tile, 512 threads, one CTA per SM | 2 = 128x32 tile, 256 threads,
