@@ -637,6 +637,14 @@ int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, i
     }
     cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e = cudaSuccess;
+    if (wavelet == IDG_WAVELET_HAAR && levels <= 3 && ny <= 65535 * 8 && nz <= 65535 * 8 &&
+        g_opt[IDG_OPT_KERNEL] != 1) {          // Haar blocks are independent: one fused pass (option kernel = 1: per-axis passes)
+        e = idg::launch_haar_filter(cube, out, nx, ny, nz, levels, thr, st);
+        if (e != cudaSuccess) return (int)e;
+        t_launches = 1;
+        snprintf(t_plan, sizeof(t_plan), "idg_haar_filter_kernel levels=%d", levels);
+        return IDG_OK;
+    }
     if ((const float *)out != cube) e = cudaMemcpyAsync(out, cube, N * sizeof(float), cudaMemcpyDeviceToDevice, st);
     int launches = 0;
     if (e == cudaSuccess) e = idg::launch_wavelet_transform(out, nx, ny, nz, wavelet, levels, false, st, &launches);

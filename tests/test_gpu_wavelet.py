@@ -79,6 +79,27 @@ def test_filter(B, oracle, shape, wavelet, thr):
         assert np.abs(out - oracle.wavelet_filter_oracle(a, wavelet, [float(np.float32(t)) for t in thr], rms)).max() <= TOL * rms
 
 
+@pytest.mark.parametrize("shape", SHAPES + [(8, 8, 32), (17, 23, 77), (64, 72, 160)], ids=IDS)
+def test_haar_fused_pass_equals_per_axis_passes(B, shape):
+    """The single-pass Haar filter (8^3 blocks in shared memory) applies the same operations in the same order as
+    the per-level, per-axis kernels: bit-identical for every shape (odd extents, regions hanging over the faces),
+    1..3 levels, in place or not."""
+    a = torch.from_numpy(noisy(shape, 23)).cuda()
+    for thr in ((0.7,), (0.5, 0.8), (0.5, 0.8, 1.1), (0.0, 0.0, 0.0)):
+        B.idg_set_option(B.IDG_OPT_KERNEL, 1)
+        try:
+            ref = B.idg_wavelet_filter(a, B.WAVELET_HAAR, thr, 1.3)
+            plan_ref = B.idg_last_plan()
+        finally:
+            B.idg_set_option(B.IDG_OPT_KERNEL, 0)
+        out = B.idg_wavelet_filter(a, B.WAVELET_HAAR, thr, 1.3)
+        assert "idg_haar_filter_kernel" in B.idg_last_plan() and "idg_lift_kernel" in plan_ref
+        assert torch.equal(out, ref), (shape, thr)
+        inplace = a.clone()
+        B.idg_wavelet_filter(inplace, B.WAVELET_HAAR, thr, 1.3, out=inplace)
+        assert torch.equal(inplace, ref)
+
+
 def test_filter_limits_and_config0(B, oracle):
     from paper_1609_03782_b200 import synth
     c = synth.modelb_like(seed=1000, snr=32.0)
