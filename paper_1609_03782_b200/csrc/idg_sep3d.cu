@@ -67,12 +67,15 @@ __global__ void __launch_bounds__(NT, Geo<RXY, RZ>::kMinBlocks) idg_sep3d_kernel
 
     // Tile loads: warp w takes halo rows w, w+8, ...; lane l takes halo columns l, l+32, (l+64) of a row.
     // Clamped global x and row offsets do not change from plane to plane.
-    int gxo[G::COL_IT];
+    // 32-bit element offsets inside a plane (the launcher rejects planes of 2^32 voxels and more), so a load
+    // is plane base (uniform) + offset
+    unsigned off[G::ROW_IT][G::COL_IT];
 #pragma unroll
-    for (int c = 0; c < G::COL_IT; ++c) gxo[c] = min(max(x0 - RXY + lane + 32 * c, 0), S.nx - 1);
-    size_t gyo[G::ROW_IT];
+    for (int i = 0; i < G::ROW_IT; ++i)
 #pragma unroll
-    for (int i = 0; i < G::ROW_IT; ++i) gyo[i] = (size_t)min(max(y0 - RXY + warp + 8 * i, 0), S.ny - 1) * (size_t)S.nx;
+        for (int c = 0; c < G::COL_IT; ++c)
+            off[i][c] = (unsigned)min(max(y0 - RXY + warp + 8 * i, 0), S.ny - 1) * (unsigned)S.nx +
+                        (unsigned)min(max(x0 - RXY + lane + 32 * c, 0), S.nx - 1);
 
     float pre[G::ROW_IT * G::COL_IT];
     auto fetch = [&](int q) {                         // plane clamp(q) -> registers
@@ -81,7 +84,7 @@ __global__ void __launch_bounds__(NT, Geo<RXY, RZ>::kMinBlocks) idg_sep3d_kernel
         for (int i = 0; i < G::ROW_IT; ++i)
 #pragma unroll
             for (int c = 0; c < G::COL_IT; ++c)
-                if (32 * c + 31 < G::COLS || lane + 32 * c < G::COLS) pre[i * G::COL_IT + c] = __ldg(src + gyo[i] + gxo[c]);
+                if (32 * c + 31 < G::COLS || lane + 32 * c < G::COLS) pre[i * G::COL_IT + c] = __ldg(src + off[i][c]);
     };
     float *a_thr = A + warp * G::STRIDE + G::OFF + lane;
     auto stash = [&]() {                              // registers -> A
@@ -246,7 +249,8 @@ cudaError_t launch_sep3d(const float *in, float *out, int nx, int ny, int nz, in
     }
     S.zchunk = (nz + chunks - 1) / chunks;
     chunks = (nz + S.zchunk - 1) / S.zchunk;
-    if (tiles_y > 65535 || chunks > 65535) return cudaErrorInvalidValue;
+    if (tiles_y > 65535 || chunks > 65535 || (unsigned long long)nx * (unsigned long long)ny >= (1ull << 32))
+        return cudaErrorInvalidValue;
     const dim3 grid((unsigned)tiles_x, (unsigned)tiles_y, (unsigned)chunks);
     switch (cxy) {
     case 0: return launch_rz<0>(cz, S, grid, st);
