@@ -317,7 +317,7 @@ int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
     if (slabs == 0) {
         slabs = 1;
         if (bytes >= (64u << 20) && n_iter > 0) {
-            const int thick = 4 * n_iter > 16 ? 4 * n_iter : 16;       // keep the halo overhead below ~50 %
+            const int thick = 3 * n_iter > 16 ? 3 * n_iter : 16;       // keep the halo overhead below ~70 %
             slabs = nz / thick;
             if (slabs > 8) slabs = 8;
             if (slabs < 1) slabs = 1;
