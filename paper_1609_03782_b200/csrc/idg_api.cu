@@ -613,7 +613,7 @@ int idg_wavelet_transform(const float *cube, int nx, int ny, int nz, int wavelet
     cudaError_t e = cudaSuccess;
     if ((const float *)out != cube) e = cudaMemcpyAsync(out, cube, N * sizeof(float), cudaMemcpyDeviceToDevice, st);
     int launches = 0;
-    if (e == cudaSuccess) e = idg::launch_wavelet_transform(out, nx, ny, nz, wavelet, levels, inverse != 0, st, &launches);
+    if (e == cudaSuccess) e = idg::launch_wavelet_transform(out, nx, ny, nz, wavelet, levels, inverse != 0, g_opt[IDG_OPT_KERNEL] == 1, st, &launches);
     if (e != cudaSuccess) return (int)e;
     t_launches = launches;
     snprintf(t_plan, sizeof(t_plan), "idg_lift_kernel %s levels=%d %s", wavelet == 0 ? "haar" : "legall53", levels,
@@ -647,9 +647,9 @@ int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, i
     }
     if ((const float *)out != cube) e = cudaMemcpyAsync(out, cube, N * sizeof(float), cudaMemcpyDeviceToDevice, st);
     int launches = 0;
-    if (e == cudaSuccess) e = idg::launch_wavelet_transform(out, nx, ny, nz, wavelet, levels, false, st, &launches);
+    if (e == cudaSuccess) e = idg::launch_wavelet_transform(out, nx, ny, nz, wavelet, levels, false, g_opt[IDG_OPT_KERNEL] == 1, st, &launches);
     if (e == cudaSuccess) { e = idg::launch_wavelet_threshold(out, nx, ny, nz, levels, thr, st); ++launches; }
-    if (e == cudaSuccess) e = idg::launch_wavelet_transform(out, nx, ny, nz, wavelet, levels, true, st, &launches);
+    if (e == cudaSuccess) e = idg::launch_wavelet_transform(out, nx, ny, nz, wavelet, levels, true, g_opt[IDG_OPT_KERNEL] == 1, st, &launches);
     if (e != cudaSuccess) return (int)e;
     t_launches = launches;
     snprintf(t_plan, sizeof(t_plan), "idg_lift_kernel %s levels=%d filter", wavelet == 0 ? "haar" : "legall53", levels);

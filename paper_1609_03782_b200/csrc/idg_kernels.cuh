@@ -129,7 +129,7 @@ cudaError_t launch_cube_stats(const float *cube, int nx, int ny, const int roi[6
 
 // Wavelet lifting (section 3.4, Eq. 8-11): in-place transform and hard thresholding.
 cudaError_t launch_wavelet_transform(float *a, int nx, int ny, int nz, int wavelet, int levels, bool inverse,
-                                     cudaStream_t st, int *launches);
+                                     bool two_phase, cudaStream_t st, int *launches);
 cudaError_t launch_haar_filter(const float *in, float *out, int nx, int ny, int nz, int levels, const float *thr,
                                cudaStream_t st);
 cudaError_t launch_wavelet_threshold(float *a, int nx, int ny, int nz, int levels, const float *thr, cudaStream_t st);

@@ -115,6 +115,93 @@ __global__ void __launch_bounds__(NT) idg_wavelet_threshold_kernel(const __grid_
     }
 }
 
+// ---- whole lines in shared memory: predict + update of one axis in ONE in-place pass ----------------------
+// A CTA that holds complete lines can run both lifting phases without another CTA touching its samples, so the
+// pass is race-free in place (what the two-phase kernels buy with a second launch).  x lines: one warp per
+// line.  y / z lines: a CTA takes 32 neighbouring lattice columns (lane = column, coalesced for level 1) and
+// the full line of each.  Same operations in the same order as idg_lift_kernel.
+template <int WAVELET, bool INV>
+__device__ __forceinline__ void lift_line_smem(float *v, int m, int stride, int first, int step, bool block_sync)
+{
+    // v[j * stride]: sample j of the line; this thread handles pair / even indices first, first+step, ...
+    const int no = m / 2, ne = m - no;
+    auto sync = [&]() { if (block_sync) __syncthreads(); else __syncwarp(); };
+    auto predict = [&]() {
+        for (int i = first; i < no; i += step) {
+            const float e0 = v[(2 * i) * stride];
+            float p = e0;
+            if (WAVELET == 1) p = 0.5f * (e0 + ((i + 1 < ne) ? v[(2 * i + 2) * stride] : e0));
+            float &d = v[(2 * i + 1) * stride];
+            d = INV ? d + p : d - p;
+        }
+    };
+    auto update = [&]() {
+        for (int i = first; i < ne; i += step) {
+            float u;
+            if (WAVELET == 0) {
+                if (i >= no) continue;
+                u = 0.5f * v[(2 * i + 1) * stride];
+            } else {
+                const float dr = (i < no) ? v[(2 * i + 1) * stride] : v[(2 * i - 1) * stride];
+                const float dl = (i > 0) ? v[(2 * i - 1) * stride] : dr;
+                u = 0.25f * (dl + dr);
+            }
+            float &c = v[(2 * i) * stride];
+            c = INV ? c - u : c + u;
+        }
+    };
+    if (!INV) { predict(); sync(); update(); } else { update(); sync(); predict(); }
+    sync();
+}
+
+constexpr int LW = 4;        // warps (= x lines) per CTA of the x-line kernel
+
+template <int WAVELET, bool INV>
+__global__ void __launch_bounds__(LW * 32) idg_lift_xline_kernel(const __grid_constant__ WArgs W)
+{
+    extern __shared__ float lsm[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float *v = lsm + (size_t)warp * W.mx;
+    const long long lines = (long long)W.my * W.mz;
+    for (long long l = (long long)blockIdx.x * LW + warp; l < lines; l += (long long)gridDim.x * LW) {
+        const int cy = (int)(l % W.my), cz = (int)(l / W.my);
+        float *g = W.a + ((size_t)cz * W.s * W.ny + (size_t)cy * W.s) * (size_t)W.nx;
+        for (int j = lane; j < W.mx; j += 32) v[j] = g[(size_t)j * W.s];
+        __syncwarp();
+        lift_line_smem<WAVELET, INV>(v, W.mx, 1, lane, 32, false);
+        for (int j = lane; j < W.mx; j += 32) g[(size_t)j * W.s] = v[j];
+        __syncwarp();
+    }
+}
+
+// axis 1 (y) or 2 (z): strip of SW lattice-x columns, full lines; smem [m][SW]
+constexpr int SW = 16;
+template <int WAVELET, bool INV>
+__global__ void __launch_bounds__(NT) idg_lift_strip_kernel(const __grid_constant__ WArgs W)
+{
+    extern __shared__ float lsm[];
+    const int col = threadIdx.x % SW, row = threadIdx.x / SW;
+    constexpr int ROWS = NT / SW;
+    const int m = W.axis == 1 ? W.my : W.mz;                      // line length
+    const int mo = W.axis == 1 ? W.mz : W.my;                     // lattice extent of the third axis
+    const int strips = (W.mx + SW - 1) / SW;
+    const size_t sline = W.axis == 1 ? (size_t)W.s * W.nx : (size_t)W.s * W.nx * (size_t)W.ny;     // along the line
+    const size_t sother = W.axis == 1 ? (size_t)W.s * W.nx * (size_t)W.ny : (size_t)W.s * W.nx;    // third axis
+    for (long long t = blockIdx.x; t < (long long)strips * mo; t += gridDim.x) {
+        const int sx = (int)(t % strips), co = (int)(t / strips);
+        const int cx = sx * SW + col;
+        const bool on = cx < W.mx;
+        float *g = W.a + (size_t)co * sother + (size_t)cx * W.s;
+        if (on)
+            for (int j = row; j < m; j += ROWS) lsm[j * SW + col] = g[(size_t)j * sline];
+        __syncthreads();
+        lift_line_smem<WAVELET, INV>(lsm + col, m, SW, row, ROWS, true);
+        if (on)
+            for (int j = row; j < m; j += ROWS) g[(size_t)j * sline] = lsm[j * SW + col];
+        __syncthreads();
+    }
+}
+
 // ---- Haar thresholding filter, up to 3 levels, in ONE pass ------------------------------------------------
 // A Haar pair never leaves its 2-block, so the whole L-level transform of an 8 x 8 x 8 aligned block depends on
 // that block only.  A CTA stages a 32 x 8 x 8 region in shared memory, runs forward levels 1..L (a thread per
@@ -264,7 +351,8 @@ cudaError_t launch_phase(const WArgs &W, cudaStream_t st)
 }
 
 template <int WAVELET>
-cudaError_t transform(float *a, int nx, int ny, int nz, int levels, bool inverse, cudaStream_t st, int *launches)
+cudaError_t transform(float *a, int nx, int ny, int nz, int levels, bool inverse, bool two_phase, cudaStream_t st,
+                      int *launches)
 {
     cudaError_t e = cudaSuccess;
     for (int li = 0; li < levels && e == cudaSuccess; ++li) {
@@ -286,6 +374,26 @@ cudaError_t transform(float *a, int nx, int ny, int nz, int levels, bool inverse
                 *launches += 1;
                 continue;
             }
+            // whole lines in shared memory: one pass per axis (falls back to two phases for very long lines)
+            const size_t line_smem = W.axis == 0 ? (size_t)LW * W.mx * sizeof(float) : (size_t)m * SW * sizeof(float);
+            if (line_smem <= 200u * 1024u && !two_phase) {
+                if (W.axis == 0) {
+                    auto k = inverse ? idg_lift_xline_kernel<WAVELET, true> : idg_lift_xline_kernel<WAVELET, false>;
+                    e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+                    long long grid = ((long long)W.my * W.mz + LW - 1) / LW;
+                    if (grid > 148LL * 16) grid = 148LL * 16;
+                    if (e == cudaSuccess) k<<<(unsigned)grid, LW * 32, line_smem, st>>>(W);
+                } else {
+                    auto k = inverse ? idg_lift_strip_kernel<WAVELET, true> : idg_lift_strip_kernel<WAVELET, false>;
+                    e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+                    long long grid = (long long)((W.mx + SW - 1) / SW) * (W.axis == 1 ? W.mz : W.my);
+                    if (grid > 148LL * 16) grid = 148LL * 16;
+                    if (e == cudaSuccess) k<<<(unsigned)grid, NT, line_smem, st>>>(W);
+                }
+                if (e == cudaSuccess) e = cudaGetLastError();
+                *launches += 1;
+                continue;
+            }
             if (!inverse) {
                 e = launch_phase<WAVELET, 0, false>(W, st);
                 if (e == cudaSuccess) e = launch_phase<WAVELET, 1, false>(W, st);
@@ -303,10 +411,10 @@ cudaError_t transform(float *a, int nx, int ny, int nz, int levels, bool inverse
 
 // In-place forward / inverse transform of `a` to `levels` (wavelet 0 Haar, 1 Le Gall 5/3).
 cudaError_t launch_wavelet_transform(float *a, int nx, int ny, int nz, int wavelet, int levels, bool inverse,
-                                     cudaStream_t st, int *launches)
+                                     bool two_phase, cudaStream_t st, int *launches)
 {
-    return wavelet == 0 ? transform<0>(a, nx, ny, nz, levels, inverse, st, launches)
-                        : transform<1>(a, nx, ny, nz, levels, inverse, st, launches);
+    return wavelet == 0 ? transform<0>(a, nx, ny, nz, levels, inverse, two_phase, st, launches)
+                        : transform<1>(a, nx, ny, nz, levels, inverse, two_phase, st, launches);
 }
 
 // Haar, 1..3 levels: the fused single-pass filter.  thr[l-1] = t_l * rms.

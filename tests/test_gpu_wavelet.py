@@ -100,6 +100,26 @@ def test_haar_fused_pass_equals_per_axis_passes(B, shape):
         assert torch.equal(inplace, ref)
 
 
+@pytest.mark.parametrize("wavelet", [0, 1], ids=["haar", "legall"])
+@pytest.mark.parametrize("shape", SHAPES + [(17, 23, 77), (64, 72, 160), (40, 300, 50)], ids=IDS)
+def test_whole_line_passes_equal_two_phase_passes(B, shape, wavelet):
+    """The one-pass-per-axis kernels (complete lines in shared memory) are bit-identical to the two-phase
+    kernels (option kernel = 1) for the transform, its inverse and the filter."""
+    a = torch.from_numpy(noisy(shape, 24)).cuda()
+    for L in (1, 2, 3, 4):
+        B.idg_set_option(B.IDG_OPT_KERNEL, 1)
+        try:
+            ref = B.idg_wavelet_transform(a, wavelet, L)
+            ref_back = B.idg_wavelet_transform(ref, wavelet, L, inverse=True)
+            ref_f = B.idg_wavelet_filter(a, wavelet, [0.4 + 0.3 * l for l in range(L)], 1.2)
+        finally:
+            B.idg_set_option(B.IDG_OPT_KERNEL, 0)
+        out = B.idg_wavelet_transform(a, wavelet, L)
+        assert torch.equal(out, ref), (shape, L)
+        assert torch.equal(B.idg_wavelet_transform(out, wavelet, L, inverse=True), ref_back)
+        assert torch.equal(B.idg_wavelet_filter(a, wavelet, [0.4 + 0.3 * l for l in range(L)], 1.2), ref_f)
+
+
 def test_filter_limits_and_config0(B, oracle):
     from paper_1609_03782_b200 import synth
     c = synth.modelb_like(seed=1000, snr=32.0)
