@@ -77,3 +77,26 @@ def cube_stats_oracle(cube: np.ndarray, roi: Optional[Sequence[int]] = None) -> 
     n, s1, s2 = int(a.size), float(a.sum()), float((a * a).sum())
     rms = math.sqrt(max(s2 / n - (s1 / n) ** 2, 0.0)) if n else math.nan
     return {"n": n, "sum": s1, "sumsq": s2, "rms": rms}
+
+
+def histogram_oracle(cube: np.ndarray, lo: float, hi: float, nbins: int,
+                     roi: Optional[Sequence[int]] = None, mask_thr: Optional[float] = None) -> np.ndarray:
+    """Histogram of the voxel intensities of a ROI sub-cube (Fig. 6; the F-versus-threshold
+    scan of PAPER.md:342 needs it).  Reading Q5: nbins equal bins over [lo, hi); the bin of a voxel is decided
+    in fp32 like the mask of Eq. 14: b = floor((v - lo) * (nbins / (hi - lo))) with every operand and operation
+    in fp32; voxels outside [lo, hi) and NaN are not counted; with mask_thr only voxels v >= mask_thr count."""
+    a = np.asarray(cube, dtype=np.float32)
+    a = a[_roi(a.shape, roi)].ravel()
+    lo32, hi32 = np.float32(lo), np.float32(hi)
+    if not (hi32 > lo32) or nbins < 1:
+        raise ValueError("need hi > lo and nbins >= 1")
+    scale = np.float32(np.float32(nbins) / np.float32(hi32 - lo32))
+    counts = np.zeros(int(nbins), dtype=np.int64)
+    keep = (a >= lo32) & (a < hi32)
+    if mask_thr is not None:
+        keep &= a >= np.float32(mask_thr)
+    v = a[keep]
+    b = np.floor((v - lo32).astype(np.float32) * scale).astype(np.int64)
+    b = np.minimum(b, nbins - 1)                         # (v - lo) * scale can round up to nbins just below hi
+    np.add.at(counts, b, 1)
+    return counts

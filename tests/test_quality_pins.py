@@ -113,3 +113,20 @@ def test_q8_rms_estimate(Q):
     assert st["n"] == sub.size and st["sum"] == pytest.approx(sub.sum(), rel=1e-14)
     assert st["rms"] == pytest.approx(np.std(sub), rel=1e-12)              # library routine
     assert Q.cube_stats_oracle(np.full((3, 3, 3), 7.0, np.float32))["rms"] == 0.0
+
+
+def test_q9_histogram(Q):
+    """Reading Q5: equal bins over [lo, hi), fp32 bin decision, out-of-range and NaN voxels dropped."""
+    a = np.array([[[-1.0, 0.0, 0.24, 0.25, 0.5, 0.99, 1.0, np.nan, 0.75, 0.7499999]]], dtype=np.float32)
+    h = Q.histogram_oracle(a, 0.0, 1.0, 4)
+    assert h.tolist() == [2, 1, 2, 2]                      # [0,.25): 0, .24 | [.25,.5): .25 | [.5,.75): .5, .7499999 | [.75,1): .99, .75
+    assert Q.histogram_oracle(a, 0.0, 1.0, 4, mask_thr=0.5).tolist() == [0, 0, 2, 2]
+    rng = np.random.default_rng(9)
+    b = rng.normal(0, 1, (6, 7, 8)).astype(np.float32)
+    h = Q.histogram_oracle(b, -4.0, 4.0, 64, roi=(1, 7, 0, 7, 2, 6))
+    sub = b[2:6, 0:7, 1:7]
+    ref, _ = np.histogram(sub, bins=64, range=(-4.0, 4.0))           # library routine (bins exactly representable)
+    inside = ((sub >= -4.0) & (sub < 4.0)).sum()
+    assert h.sum() == inside and np.array_equal(h, ref)
+    with pytest.raises(ValueError):
+        Q.histogram_oracle(b, 1.0, 1.0, 4)
