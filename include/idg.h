@@ -205,6 +205,15 @@ int idg_mask_sums(const float *orig, const float *filt, const float *model, int 
 int idg_cube_stats(const float *cube, int nx, int ny, int nz, const idg_roi *roi, double *stats, void *stream);
 
 /*
+ * Histogram of the voxel intensities of the ROI (Fig. 6): `nbins` (1..8192) equal bins over
+ * [lo, hi); a voxel v with lo <= v < hi (and v >= *mask_thr when mask_thr is given) counts in bin
+ * floor((v - lo) * (nbins / (hi - lo))), every operation in fp32 (reading Q5); NaN never counts.
+ *   cube [device];  mask_thr [host] one float or NULL;  counts [device] nbins 64-bit counters, overwritten
+ */
+int idg_histogram(const float *cube, int nx, int ny, int nz, const idg_roi *roi, float lo, float hi, int nbins,
+                  const float *mask_thr, unsigned long long *counts, void *stream);
+
+/*
  * Host-only: F = |S_of|/|S_oo| (Eq. 12), its error (Eq. 15-16, with N_i = population / voxels_per_beam,
  * voxels_per_beam >= 1) and F_M = |S_mf|/|S_m| (Eq. 17) from a HOST copy of the sums.  Any of the three
  * output pointers may be NULL; a ratio with a zero denominator is NaN.

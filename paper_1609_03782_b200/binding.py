@@ -26,7 +26,7 @@ SYMBOLS = ("idg_version", "idg_status_string", "idg_params_check", "idg_workspac
            "idg_set_option", "idg_get_option", "idg_last_launch_count", "idg_last_plan",
            "idg_box_filter", "idg_gaussian_filter", "idg_gaussian_radii",
            "idg_mask_sums", "idg_cube_stats", "idg_quality", "idg_filter_pm",
-           "idg_wavelet_transform", "idg_wavelet_filter")
+           "idg_wavelet_transform", "idg_wavelet_filter", "idg_histogram")
 WAVELET_HAAR, WAVELET_LEGALL53 = 0, 1
 
 
@@ -113,6 +113,8 @@ def lib() -> ctypes.CDLL:
         L.idg_mask_sums.argtypes = [fp, fp, fp, i, i, i, rp, f, f, vp, vp]
         L.idg_cube_stats.restype = i
         L.idg_cube_stats.argtypes = [fp, i, i, i, rp, vp, vp]
+        L.idg_histogram.restype = i
+        L.idg_histogram.argtypes = [fp, i, i, i, rp, f, f, i, ctypes.POINTER(ctypes.c_float), vp, vp]
         L.idg_quality.restype = i
         L.idg_quality.argtypes = [dptr, d, d, d, dptr, dptr, dptr]
         L.idg_wavelet_transform.restype = i
@@ -332,6 +334,19 @@ def idg_cube_stats(cube: torch.Tensor, roi=None, stats: Optional[torch.Tensor] =
     _check(lib().idg_cube_stats(_dev(cube, "cube"), nx, ny, nz, None if r is None else ctypes.byref(r),
                                 stats.data_ptr(), _stream(stream)))
     return stats
+
+
+def idg_histogram(cube: torch.Tensor, lo: float, hi: float, nbins: int, roi=None, mask_thr: Optional[float] = None,
+                  counts: Optional[torch.Tensor] = None, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """idg_histogram: device tensor of nbins int64 counts over [lo, hi) for the ROI."""
+    nz, ny, nx = cube.shape
+    if counts is None:
+        counts = torch.empty(int(nbins), dtype=torch.int64, device=cube.device)
+    r = _roi(roi)
+    thr = None if mask_thr is None else ctypes.byref(ctypes.c_float(float(mask_thr)))
+    _check(lib().idg_histogram(_dev(cube, "cube"), nx, ny, nz, None if r is None else ctypes.byref(r), float(lo),
+                               float(hi), int(nbins), thr, counts.data_ptr(), _stream(stream)))
+    return counts
 
 
 def idg_quality(sums: Sequence[float], rms_o: float, rms_f: float, voxels_per_beam: float = 1.0) -> dict:

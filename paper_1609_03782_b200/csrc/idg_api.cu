@@ -573,6 +573,26 @@ int idg_cube_stats(const float *cube, int nx, int ny, int nz, const idg_roi *roi
     return IDG_OK;
 }
 
+int idg_histogram(const float *cube, int nx, int ny, int nz, const idg_roi *roi, float lo, float hi, int nbins,
+                  const float *mask_thr, unsigned long long *counts, void *stream)
+{
+    t_launches = 0;
+    if (!(hi > lo) || !isfinite(lo) || !isfinite(hi) || nbins < 1 || nbins > 8192 || (mask_thr && isnan(*mask_thr)))
+        return IDG_ERR_PARAM;
+    if (!cube || !counts) return IDG_ERR_NULL;
+    size_t N;
+    if (!voxel_count(nx, ny, nz, 1, &N)) return IDG_ERR_DIMS;
+    if (((uintptr_t)counts & 7u) != 0) return IDG_ERR_WORKSPACE;
+    int r[6];
+    const int rc = roi_box(roi, nx, ny, nz, r);
+    if (rc != IDG_OK) return rc;
+    const cudaError_t e = idg::launch_histogram(cube, nx, ny, r, lo, hi, nbins, mask_thr, counts, (cudaStream_t)stream);
+    if (e != cudaSuccess) return (int)e;
+    t_launches = 1;
+    snprintf(t_plan, sizeof(t_plan), "idg_histogram_kernel nbins=%d", nbins);
+    return IDG_OK;
+}
+
 int idg_quality(const double *sums, double rms_o, double rms_f, double voxels_per_beam, double *F, double *sigma_F,
                 double *F_M)
 {

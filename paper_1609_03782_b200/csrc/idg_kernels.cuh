@@ -125,6 +125,8 @@ cudaError_t launch_conv3d(const float *in, float *out, int nx, int ny, int nz, i
 cudaError_t launch_mask_sums(const float *o, const float *f, const float *m, int nx, int ny, const int roi[6],
                              float thr_o, float thr_f, double *out, cudaStream_t st);
 cudaError_t launch_cube_stats(const float *cube, int nx, int ny, const int roi[6], double *out, cudaStream_t st);
+cudaError_t launch_histogram(const float *cube, int nx, int ny, const int roi[6], float lo, float hi, int nbins,
+                             const float *mask_thr, unsigned long long *counts, cudaStream_t st);
 
 
 // Wavelet lifting (section 3.4, Eq. 8-11): in-place transform and hard thresholding.

@@ -113,6 +113,44 @@ __global__ void __launch_bounds__(NT) idg_cube_stats_kernel(const __grid_constan
     }
 }
 
+// Intensity histogram of a ROI (Fig. 6; reading Q5): nbins equal bins over [lo, hi), bin
+// decided in fp32 as floor((v - lo) * scale) with scale = nbins / (hi - lo) rounded to fp32 on the host (no FMA
+// contraction, so that the integer decision is the oracle's), per-CTA counts in shared memory, merged with one
+// 64-bit atomic per non-empty bin.
+struct HistArgs {
+    const float *a;
+    int nx, ny;
+    int x0, x1, y0, y1, z0, z1;
+    float lo, hi, scale, thr;
+    int use_thr, nbins;
+    unsigned long long *counts;
+};
+
+__global__ void __launch_bounds__(NT) idg_histogram_kernel(const __grid_constant__ HistArgs H)
+{
+    extern __shared__ unsigned hist[];
+    for (int b = threadIdx.x; b < H.nbins; b += NT) hist[b] = 0u;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int rows_y = H.y1 - H.y0;
+    const long long rows = (long long)rows_y * (H.z1 - H.z0);
+    for (long long r = (long long)blockIdx.x * WARPS + warp; r < rows; r += (long long)gridDim.x * WARPS) {
+        const int z = H.z0 + (int)(r / rows_y), y = H.y0 + (int)(r % rows_y);
+        const float *row = H.a + ((size_t)z * H.ny + y) * (size_t)H.nx;
+        for (int x = H.x0 + lane; x < H.x1; x += 32) {
+            const float v = row[x];
+            if (v >= H.lo && v < H.hi && (!H.use_thr || v >= H.thr)) {
+                int b = (int)floorf(__fmul_rn(__fsub_rn(v, H.lo), H.scale));
+                b = b < H.nbins - 1 ? b : H.nbins - 1;
+                atomicAdd(&hist[b], 1u);
+            }
+        }
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < H.nbins; b += NT)
+        if (hist[b]) atomicAdd(H.counts + b, (unsigned long long)hist[b]);
+}
+
 unsigned grid_for(long long rows)
 {
     long long g = (rows + WARPS - 1) / WARPS;
@@ -136,6 +174,20 @@ cudaError_t launch_mask_sums(const float *o, const float *f, const float *m, int
     if (rows <= 0 || roi[1] <= roi[0]) return cudaSuccess;   // empty ROI: all sums zero
     if (m) idg_mask_sums_kernel<true><<<grid_for(rows), NT, 0, st>>>(Q);
     else idg_mask_sums_kernel<false><<<grid_for(rows), NT, 0, st>>>(Q);
+    return cudaGetLastError();
+}
+
+// counts [device] nbins 64-bit counters, zeroed here.  A CTA sees fewer than 2^32 voxels (grid-stride over rows).
+cudaError_t launch_histogram(const float *cube, int nx, int ny, const int roi[6], float lo, float hi, int nbins,
+                             const float *mask_thr, unsigned long long *counts, cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(counts, 0, (size_t)nbins * sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return e;
+    HistArgs H{cube, nx, ny, roi[0], roi[1], roi[2], roi[3], roi[4], roi[5], lo, hi, (float)nbins / (hi - lo),
+               mask_thr ? *mask_thr : 0.f, mask_thr ? 1 : 0, nbins, counts};
+    const long long rows = (long long)(roi[3] - roi[2]) * (roi[5] - roi[4]);
+    if (rows <= 0 || roi[1] <= roi[0]) return cudaSuccess;
+    idg_histogram_kernel<<<grid_for(rows), NT, (size_t)nbins * sizeof(unsigned), st>>>(H);
     return cudaGetLastError();
 }
 

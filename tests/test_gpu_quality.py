@@ -81,6 +81,23 @@ def test_quality_on_a_filtered_config0_cube(B, Q, oracle):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("shape", [(1, 1, 1), (3, 5, 7), (17, 40, 132), (6, 50, 100)], ids=lambda s: "x".join(map(str, s[::-1])))
+def test_histogram_is_bit_exact(B, Q, shape):
+    """Integer work: every count must equal the oracle's (the bin is decided in fp32 on both sides)."""
+    rng = np.random.default_rng(sum(shape) + 3)
+    a = (rng.normal(0, 1, shape) + 6.0 * (rng.random(shape) < 0.1)).astype(np.float32)
+    a.flat[0] = np.float32(-4.0)                      # on the lower edge: counted;  upper edge: not
+    if a.size > 1:
+        a.flat[1] = np.float32(4.0)
+    t = torch.from_numpy(a).cuda()
+    nz, ny, nx = shape
+    for lo, hi, nb, roi, thr in ((-4.0, 4.0, 64, None, None), (-0.3, 7.1, 37, None, None), (-4.0, 4.0, 1, None, None),
+                                 (0.0, 10.0, 1000, (nx // 3, nx, 0, ny, nz // 2, nz), None), (-4.0, 4.0, 64, None, 0.5)):
+        got = B.idg_histogram(t, lo, hi, nb, roi, thr).cpu().numpy()
+        assert np.array_equal(got, Q.histogram_oracle(a, lo, hi, nb, roi, thr)), (lo, hi, nb, roi, thr)
+
+
+@pytest.mark.gpu
 def test_argument_errors(B):
     a = torch.zeros((4, 5, 8), device="cuda")
     with pytest.raises(B.IdgError) as e:
@@ -91,6 +108,10 @@ def test_argument_errors(B):
     assert e.value.status == -4
     with pytest.raises(TypeError):
         B.idg_cube_stats(a.cpu())
+    for lo, hi, nb in ((1.0, 1.0, 4), (0.0, 1.0, 0), (0.0, 1.0, 9000), (float("nan"), 1.0, 4)):
+        with pytest.raises(B.IdgError) as e:
+            B.idg_histogram(a, lo, hi, nb)
+        assert e.value.status == -4
 
 
 def test_idg_quality_host_formulas(B, Q):
