@@ -128,3 +128,16 @@ def test_idg_quality_host_formulas(B, Q):
         B.idg_quality(sums, 0.0, 1.0)
     with pytest.raises(B.IdgError):
         B.idg_quality(sums, 1.0, 1.0, voxels_per_beam=0.5)
+
+
+@pytest.mark.gpu
+def test_parameter_exploration_runs_and_behaves_like_the_paper(B):
+    """explore.py: the config-1 sweep with on-device diagnostics.  Soft checks from the paper: smoothing lowers the
+    noise monotonically with n, and the adaptive filter lifts faint signal above 3 rms (F > 1)
+    while recovering a growing share of the model flux (F_M grows with F)."""
+    from paper_1609_03782_b200 import explore
+    rows = explore.explore(snr=22.0, seed=1001, nmax=20, ks=(1.5,), report=(1, 5, 10, 20))
+    assert [r["n"] for r in rows] == [1, 5, 10, 20]
+    rms = [r["rms_f"] for r in rows]
+    assert all(a > b for a, b in zip(rms, rms[1:])) and rms[-1] < 0.5
+    assert rows[-1]["F"] > 1.0 and rows[-1]["F_M"] > rows[0]["F_M"] and all(r["sigma_F"] > 0 for r in rows)
