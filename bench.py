@@ -374,7 +374,7 @@ def run_ours(args) -> None:
     }
     if filt is None:
         # after temporal fusion the IDG kernels sit between the DRAM and the FP32 ceilings: report the second too
-        lane_ops = 12.0 * value * 1e9 / 1e12                       # 12 FP32 lane-ops per voxel-iteration
+        lane_ops = 10.0 * value * 1e9 / 1e12                       # 10 FP32 lane-ops per voxel-iteration
         peak_ops = 148 * 128 * 1.965e9 / 1e12
         line["roofline"]["alu"] = {"achieved": lane_ops, "peak": peak_ops, "unit": "T lane-op/s", "frac": lane_ops / peak_ops,
                                    "note": "useful voxel-iterations only; halo recomputation (x 1.3-1.4) comes on top"}

@@ -49,6 +49,7 @@ idg::CubeParams prepare(const idg_params &p, int n_iter)
     c.ay = (float)((double)p.tau * (double)p.cy);
     c.az = (float)((double)p.tau * (double)p.cz);
     c.s = isinf(p.K) ? 0.0f : (float)(1.0 / ((double)p.K * (double)p.rms));
+    c.w = (float)(-2.0 * (double)p.tau * ((double)p.cx + (double)p.cy + (double)p.cz));
     c.n_iter = n_iter;
     return c;
 }

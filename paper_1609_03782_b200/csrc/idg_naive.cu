@@ -28,8 +28,8 @@ __global__ void __launch_bounds__(256) idg_naive_kernel(const __grid_constant__ 
         const float yp = y < L.ny - 1 ? src[i + L.nx] : c;
         const float zm = z > 0 ? src[i - plane] : c;
         const float zp = z < L.nz - 1 ? src[i + plane] : c;
-        dst[i] = L.mode == 1 ? update_pm(c, xm, xp, ym, yp, zm, zp, p.ax, p.ay, p.az, p.s)
-                             : update(c, xm, xp, ym, yp, zm, zp, p.ax, p.ay, p.az, p.s);
+        dst[i] = L.mode == 1 ? update_pm(c, xm, xp, ym, yp, zm, zp, p.ax, p.ay, p.az, p.s, p.w)
+                             : update(c, xm, xp, ym, yp, zm, zp, p.ax, p.ay, p.az, p.s, p.w);
     }
 }
 

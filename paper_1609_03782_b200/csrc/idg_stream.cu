@@ -57,11 +57,11 @@ __device__ __forceinline__ F4 ld4(uint32_t a)
 
 // Four voxel updates of one float4 column with packed fp32x2 arithmetic.  Each component rounds
 // exactly like the scalar update() of idg_kernels.cuh (same operations in the same order).
-struct Consts { float2 m2, ax, ay, az, s, one; };
-__device__ __forceinline__ Consts make_consts(float ax, float ay, float az, float s)
+struct Consts { float2 w, ax, ay, az, s, one; };
+__device__ __forceinline__ Consts make_consts(float ax, float ay, float az, float s, float w)
 {
     Consts k;
-    k.m2 = make_float2(-2.0f, -2.0f);
+    k.w = make_float2(w, w);
     k.ax = make_float2(ax, ax);
     k.ay = make_float2(ay, ay);
     k.az = make_float2(az, az);
@@ -72,10 +72,8 @@ __device__ __forceinline__ Consts make_consts(float ax, float ay, float az, floa
 __device__ __forceinline__ float2 update2(float2 c, float2 sx, float2 ym, float2 yp, float2 zm, float2 zp,
                                           const Consts &k)
 {
-    const float2 dx = __ffma2_rn(k.m2, c, sx);
-    const float2 dy = __ffma2_rn(k.m2, c, __fadd2_rn(yp, ym));
-    const float2 dz = __ffma2_rn(k.m2, c, __fadd2_rn(zp, zm));
-    const float2 lap = __ffma2_rn(k.az, dz, __ffma2_rn(k.ay, dy, __fmul2_rn(k.ax, dx)));
+    const float2 lap = __ffma2_rn(k.ax, sx, __ffma2_rn(k.ay, __fadd2_rn(yp, ym),
+                                                        __ffma2_rn(k.az, __fadd2_rn(zp, zm), __fmul2_rn(k.w, c))));
     const float2 u = __fmul2_rn(c, k.s);
     const float2 den = __ffma2_rn(u, u, k.one);
     const float2 r = make_float2(rcp_approx(den.x), rcp_approx(den.y));
@@ -87,10 +85,8 @@ __device__ __forceinline__ float2 update2_pm(float2 c, float2 sx, float2 gx, flo
                                              float2 zp, const Consts &k)
 {
     const float2 neg = make_float2(-1.0f, -1.0f);
-    const float2 dx = __ffma2_rn(k.m2, c, sx);
-    const float2 dy = __ffma2_rn(k.m2, c, __fadd2_rn(yp, ym));
-    const float2 dz = __ffma2_rn(k.m2, c, __fadd2_rn(zp, zm));
-    const float2 lap = __ffma2_rn(k.az, dz, __ffma2_rn(k.ay, dy, __fmul2_rn(k.ax, dx)));
+    const float2 lap = __ffma2_rn(k.ax, sx, __ffma2_rn(k.ay, __fadd2_rn(yp, ym),
+                                                        __ffma2_rn(k.az, __fadd2_rn(zp, zm), __fmul2_rn(k.w, c))));
     const float2 gy = __ffma2_rn(neg, ym, yp), gz = __ffma2_rn(neg, zm, zp);
     const float2 G = __ffma2_rn(gz, gz, __ffma2_rn(gy, gy, __fmul2_rn(gx, gx)));
     const float2 den = __ffma2_rn(k.s, G, k.one);
@@ -221,7 +217,7 @@ struct Seg {
     uint32_t xo;        // byte offset of my (possibly x-mirrored) lane inside a stage row
     unsigned ok;        // bits 0..R-1: row r is stored; bit 28: first float4 of the cube row; bit 29: last
     float *po;          // where my row-0 float4 of the plane before the first output goes
-    float ax, ay, az, sc;
+    float ax, ay, az, sc, w;
 };
 
 // Entered by every warp at the start of a segment (rare): thread state, the warp's row-offset
@@ -235,7 +231,7 @@ __device__ __noinline__ void segment_setup(const Launch &L, const StreamArgs &A,
     float *dst;
     CubeParams prm;
     const SegInfo si = seg_info(L, A, cur.tile, dst, prm);
-    S.ax = prm.ax; S.ay = prm.ay; S.az = prm.az; S.sc = prm.s;
+    S.ax = prm.ax; S.ay = prm.ay; S.az = prm.az; S.sc = prm.s; S.w = prm.w;
     if (lane == 0) {
         const uint32_t a = sbase + Y::oSeg + (seg & 3u) * 16u;
         asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(si.tx0), "r"(si.ty0), "r"(si.b),
@@ -344,7 +340,7 @@ __device__ __forceinline__ void run(const Launch &L, const StreamArgs &A, const 
         const uint32_t a0 = sbase + s0 * Y::kStage + S.xo, a1 = sbase + s1 * Y::kStage + S.xo,
                        a2 = sbase + s2 * Y::kStage + S.xo;
         const bool first = (S.ok >> 28) & 1u, last = (S.ok >> 29) & 1u;
-        const Consts kc = make_consts(S.ax, S.ay, S.az, PM ? 0.25f * S.sc * S.sc : S.sc);
+        const Consts kc = make_consts(S.ax, S.ay, S.az, PM ? 0.25f * S.sc * S.sc : S.sc, S.w);
         const bool st_on = cur.q >= cur.qs;
         S.po += plane;
 

@@ -48,10 +48,10 @@ __device__ __forceinline__ F4 update4(const F4 &c, float left, float right, cons
                                       const F4 &zm, const F4 &zp, const CubeParams &p)
 {
     F4 o;
-    o.x = update(c.x, left, c.y, ym.x, yp.x, zm.x, zp.x, p.ax, p.ay, p.az, p.s);
-    o.y = update(c.y, c.x, c.z, ym.y, yp.y, zm.y, zp.y, p.ax, p.ay, p.az, p.s);
-    o.z = update(c.z, c.y, c.w, ym.z, yp.z, zm.z, zp.z, p.ax, p.ay, p.az, p.s);
-    o.w = update(c.w, c.z, right, ym.w, yp.w, zm.w, zp.w, p.ax, p.ay, p.az, p.s);
+    o.x = update(c.x, left, c.y, ym.x, yp.x, zm.x, zp.x, p.ax, p.ay, p.az, p.s, p.w);
+    o.y = update(c.y, c.x, c.z, ym.y, yp.y, zm.y, zp.y, p.ax, p.ay, p.az, p.s, p.w);
+    o.z = update(c.z, c.y, c.w, ym.z, yp.z, zm.z, zp.z, p.ax, p.ay, p.az, p.s, p.w);
+    o.w = update(c.w, c.z, right, ym.w, yp.w, zm.w, zp.w, p.ax, p.ay, p.az, p.s, p.w);
     return o;
 }
 

@@ -45,12 +45,12 @@ __device__ __forceinline__ void sts4(float *p, const F4 &a)
 // FMUL2: two IEEE fp32 results per issued instruction; each component rounds exactly like the
 // scalar update() of idg_kernels.cuh, so results are bit-identical to the scalar kernels).
 struct Consts {
-    float2 m2, ax, ay, az, s, one;
+    float2 w, ax, ay, az, s, one;
 };
 __device__ __forceinline__ Consts make_consts(const CubeParams &p)
 {
     Consts k;
-    k.m2 = make_float2(-2.0f, -2.0f);
+    k.w = make_float2(p.w, p.w);
     k.ax = make_float2(p.ax, p.ax);
     k.ay = make_float2(p.ay, p.ay);
     k.az = make_float2(p.az, p.az);
@@ -62,10 +62,8 @@ using ptx::rcp_approx;
 __device__ __forceinline__ float2 update2(float2 c, float2 sx, float2 ym, float2 yp, float2 zm, float2 zp,
                                           const Consts &k)
 {
-    const float2 dx = __ffma2_rn(k.m2, c, sx);
-    const float2 dy = __ffma2_rn(k.m2, c, __fadd2_rn(yp, ym));
-    const float2 dz = __ffma2_rn(k.m2, c, __fadd2_rn(zp, zm));
-    const float2 lap = __ffma2_rn(k.az, dz, __ffma2_rn(k.ay, dy, __fmul2_rn(k.ax, dx)));
+    const float2 lap = __ffma2_rn(k.ax, sx, __ffma2_rn(k.ay, __fadd2_rn(yp, ym),
+                                                        __ffma2_rn(k.az, __fadd2_rn(zp, zm), __fmul2_rn(k.w, c))));
     const float2 u = __fmul2_rn(c, k.s);
     const float2 den = __ffma2_rn(u, u, k.one);
     const float2 r = make_float2(rcp_approx(den.x), rcp_approx(den.y));

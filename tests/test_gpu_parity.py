@@ -267,12 +267,15 @@ def test_batched_mixed_iteration_counts(B, oracle):
 
 @pytest.mark.parametrize("plan", PLANS, ids=PLAN_IDS)
 def test_invariants_bitwise(B, plan):
-    """On the GPU output directly: constant cube fixed point, odd symmetry, power-of-two scale
-    covariance -- all bitwise in fp32."""
+    """On the GPU output directly: odd symmetry and power-of-two scale covariance are bitwise in fp32; a
+    constant cube is a fixed point up to the rounding of the expanded numerator (a few ulp after 6
+    iterations; bitwise when the weights are powers of two) -- DESIGN.md section 6."""
     set_plan(B, plan)
     p = B.Params(K=1.5, tau=0.0325, cx=5.0, cy=3.0, cz=6.0, rms=1.0)
     const = torch.full((9, 20, 36), 7.3, device="cuda")
-    assert torch.equal(B.idg_filter(const, 6, p), const)
+    assert float((B.idg_filter(const, 6, p) - const).abs().max()) <= 7.3 * 6 * 2.0 ** -23
+    p2 = B.Params(K=1.5, tau=0.03125, cx=4.0, cy=2.0, cz=1.0, rms=1.0)      # tau Cj and w exact in fp32
+    assert torch.equal(B.idg_filter(const, 6, p2), const)
     g = torch.Generator(device="cpu").manual_seed(3)
     a = (torch.randn(9, 20, 36, generator=g) * 3).cuda()
     f = B.idg_filter(a, 6, p)
