@@ -27,20 +27,21 @@ dist.init_process_group("gloo")
 rank, world = dist.get_rank(), dist.get_world_size()
 ms = 10.0 if rank == 0 else 25.0            # rank 1 is the slow one
 slow = bench.max_over_ranks(ms, world, "cpu")
-print(json.dumps({{"rank": rank, "world": world, "slow": slow,
-                  "value": bench.aggregate_value(5.0e9, world, slow)}}), flush=True)
+with open(os.path.join({out!r}, "rank%d.json" % rank), "w") as f:       # one file per rank: stdout of two ranks can interleave
+    json.dump({{"rank": rank, "world": world, "slow": slow,
+               "value": bench.aggregate_value(5.0e9, world, slow)}}, f)
 dist.destroy_process_group()
 """
 
 
 def test_max_over_ranks_and_aggregate_world2(tmp_path):
     script = tmp_path / "worker.py"
-    script.write_text(WORKER.format(root=ROOT))
+    script.write_text(WORKER.format(root=ROOT, out=str(tmp_path)))
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
            "--master-addr", "127.0.0.1", "--master-port", str(free_port()), str(script)]
     out = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT)
     assert out.returncode == 0, out.stderr[-2000:]
-    lines = [json.loads(l) for l in out.stdout.splitlines() if l.startswith("{")]
+    lines = [json.loads((tmp_path / f"rank{r}.json").read_text()) for r in (0, 1)]
     assert sorted(l["rank"] for l in lines) == [0, 1]
     for l in lines:
         assert l["world"] == 2 and l["slow"] == 25.0                    # every rank sees the slowest time
@@ -61,7 +62,7 @@ def test_reference_arm_under_torchrun_world2():
            "--warmup", "0", "--workload", "cfg0_100x100x67_n10"]
     out = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
     assert out.returncode == 0, out.stderr[-2000:]
-    lines = [json.loads(l) for l in out.stdout.splitlines() if l.startswith("{")]
+    lines = [json.loads(l) for l in out.stdout.splitlines() if l.startswith('{"')]
     assert len(lines) == 1                                               # rank 0 alone prints
     r = lines[0]
     assert r["impl"] == "reference" and r["n_gpus"] == 2 and r["unit"] == "Gvoxel-iter/s"
