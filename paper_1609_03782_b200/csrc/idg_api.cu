@@ -273,7 +273,7 @@ int idg_filter(const float *cube, int nx, int ny, int nz, int n_iter, const idg_
     if (!params_valid(*params)) return IDG_ERR_PARAM;
     cudaStream_t st = (cudaStream_t)stream;
     void *ws = nullptr;
-    cudaError_t e = cudaMallocAsync(&ws, need, st);
+    cudaError_t e = idg::temp_alloc(&ws, need, st);
     if (e != cudaSuccess) return (int)e;
     const int rc = run(cube, nx, ny, nz, 1, nullptr, n_iter, params, out, ws, need, st);
     e = cudaFreeAsync(ws, st);
@@ -300,7 +300,7 @@ int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
     if (base) {
         if (dev_buffers_bytes < need || ((uintptr_t)base % kAlign) != 0) return IDG_ERR_WORKSPACE;
     } else {
-        e = cudaMallocAsync((void **)&base, need, st);
+        e = idg::temp_alloc((void **)&base, need, st);
         if (e != cudaSuccess) return (int)e;
         own = true;
     }
@@ -514,7 +514,7 @@ int idg_gaussian_filter(const float *cube, int nx, int ny, int nz, float fwhm_x,
     std::vector<float> gf(g.size());
     for (size_t t = 0; t < g.size(); ++t) gf[t] = (float)(g[t] / sum);
     float *d_k = nullptr;
-    cudaError_t e = cudaMallocAsync((void **)&d_k, gf.size() * sizeof(float), st);
+    cudaError_t e = idg::temp_alloc((void **)&d_k, gf.size() * sizeof(float), st);
     if (e != cudaSuccess) return (int)e;
     e = cudaMemcpyAsync(d_k, gf.data(), gf.size() * sizeof(float), cudaMemcpyHostToDevice, st);   // pageable: staged before return
     if (e == cudaSuccess) e = idg::launch_conv3d(cube, out, nx, ny, nz, rr, d_k, st);
@@ -666,8 +666,21 @@ int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, i
         snprintf(t_plan, sizeof(t_plan), "idg_haar_filter_kernel levels=%d", levels);
         return IDG_OK;
     }
-    if ((const float *)out != cube) e = cudaMemcpyAsync(out, cube, N * sizeof(float), cudaMemcpyDeviceToDevice, st);
     int launches = 0;
+    if (wavelet == IDG_WAVELET_LEGALL53 && g_opt[IDG_OPT_KERNEL] == 0) {
+        // three axes of a level fused, out of place in a stream-ordered temporary (option kernel = 2: in-place
+        // passes with whole lines in shared memory, 1: two-phase in-place passes)
+        e = idg::launch_legall_filter(cube, out, nx, ny, nz, levels, thr, st, &launches);
+        if (e == cudaSuccess) {
+            t_launches = launches;
+            snprintf(t_plan, sizeof(t_plan), "idg_legall_fwd_kernel/idg_legall_inv_kernel levels=%d", levels);
+            return IDG_OK;
+        }
+        if (e != cudaErrorMemoryAllocation) return (int)e;
+        e = cudaSuccess;                       // no room for the temporary: the in-place path needs none
+        launches = 0;
+    }
+    if ((const float *)out != cube) e = cudaMemcpyAsync(out, cube, N * sizeof(float), cudaMemcpyDeviceToDevice, st);
     if (e == cudaSuccess) e = idg::launch_wavelet_transform(out, nx, ny, nz, wavelet, levels, false, g_opt[IDG_OPT_KERNEL] == 1, st, &launches);
     if (e == cudaSuccess) { e = idg::launch_wavelet_threshold(out, nx, ny, nz, levels, thr, st); ++launches; }
     if (e == cudaSuccess) e = idg::launch_wavelet_transform(out, nx, ny, nz, wavelet, levels, true, g_opt[IDG_OPT_KERNEL] == 1, st, &launches);

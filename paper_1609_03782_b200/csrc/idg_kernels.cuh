@@ -105,9 +105,16 @@ cudaError_t launch_stream(const Launch &L, int nctas, int tile, cudaStream_t st)
 bool stream_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
 
 
+// Stream-ordered temporaries (idg_tmap.cu): cudaMallocAsync from a private memory pool that keeps what it has
+// been given (release threshold = everything), so a call that needs a cube-sized temporary does not pay the
+// driver's map / unmap every time; temp_trim() hands the unused part back.  Free with cudaFreeAsync.
+cudaError_t temp_alloc(void **p, size_t bytes, cudaStream_t st);
+cudaError_t temp_trim();
+
 // Tensor maps for the TMA kernels (idg_tmap.cu): 4-D (x, y, z, cube), box tile_x x tile_y x 1 x 1, zero fill.
 bool tmap_available();
-bool tmap_encode(CUtensorMap *m, const float *base, int nx, int ny, int nz, int batch, int tile_x, int tile_y);
+bool tmap_encode(CUtensorMap *m, const float *base, int nx, int ny, int nz, int batch, int tile_x, int tile_y,
+                 int tile_z = 1);
 
 // Reference filters (PAPER.md sections 3.1-3.2): separable single-pass filter (box, axis-aligned
 // Gaussian) and dense 3-D convolution (rotated Gaussian, Eq. 3).
@@ -133,6 +140,10 @@ cudaError_t launch_wavelet_transform(float *a, int nx, int ny, int nz, int wavel
                                      bool two_phase, cudaStream_t st, int *launches);
 cudaError_t launch_haar_filter(const float *in, float *out, int nx, int ny, int nz, int levels, const float *thr,
                                cudaStream_t st);
+// idg_legall.cu: Le Gall 5/3 thresholding filter with the axes of a level fused (needs ~1.3 cubes of temporary;
+// cudaErrorMemoryAllocation with nothing launched when there is no room).
+cudaError_t launch_legall_filter(const float *in, float *out, int nx, int ny, int nz, int levels, const float *thr,
+                                 cudaStream_t st, int *launches);
 cudaError_t launch_wavelet_threshold(float *a, int nx, int ny, int nz, int levels, const float *thr, cudaStream_t st);
 
 }  // namespace idg

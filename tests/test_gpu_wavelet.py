@@ -120,6 +120,32 @@ def test_whole_line_passes_equal_two_phase_passes(B, shape, wavelet):
         assert torch.equal(B.idg_wavelet_filter(a, wavelet, [0.4 + 0.3 * l for l in range(L)], 1.2), ref_f)
 
 
+@pytest.mark.parametrize("shape", SHAPES + [(17, 23, 77), (70, 35, 67), (64, 72, 160), (40, 300, 50), (131, 19, 36)],
+                         ids=IDS)
+def test_legall_fused_levels_equal_in_place_passes(B, shape):
+    """The Le Gall filter with the three axes of a level fused (out of place, compact lattices, thresholds
+    applied on load: idg_legall.cu, the default) is bit-identical to the in-place passes (option kernel = 2:
+    whole lines in shared memory; 1: two phases), also when it runs in place, for tiles with ragged tails,
+    odd lattice extents at every level and levels deeper than the cube."""
+    a = torch.from_numpy(noisy(shape, 31)).cuda()
+    for L in (1, 2, 3, 5):
+        thr = [0.4 + 0.3 * l for l in range(L)]
+        refs = []
+        for k in (1, 2):
+            B.idg_set_option(B.IDG_OPT_KERNEL, k)
+            try:
+                refs.append(B.idg_wavelet_filter(a, B.WAVELET_LEGALL53, thr, 1.2))
+                assert "idg_lift" in B.idg_last_plan()
+            finally:
+                B.idg_set_option(B.IDG_OPT_KERNEL, 0)
+        out = B.idg_wavelet_filter(a, B.WAVELET_LEGALL53, thr, 1.2)
+        assert "idg_legall_fwd_kernel" in B.idg_last_plan() and B.idg_last_launch_count() == 2 * L
+        assert torch.equal(refs[0], refs[1]) and torch.equal(out, refs[0]), (shape, L)
+        inplace = a.clone()
+        B.idg_wavelet_filter(inplace, B.WAVELET_LEGALL53, thr, 1.2, out=inplace)
+        assert torch.equal(inplace, out)
+
+
 def test_filter_limits_and_config0(B, oracle):
     from paper_1609_03782_b200 import synth
     c = synth.modelb_like(seed=1000, snr=32.0)
