@@ -87,8 +87,8 @@ size_t idg_workspace_bytes(int nx, int ny, int nz, int batch);
 
 /*
  * n_iter IDG updates (Eq. 7) of one cube.  north_star signature: the scratch
- * cube is taken from the stream-ordered allocator (cudaMallocAsync on `stream`)
- * and returned to it before the call returns.
+ * cube is a stream-ordered temporary (see idg_release_temporaries) taken on
+ * `stream` and returned before the call returns.
  *   cube   [device] nx*ny*nz fp32, input I_0
  *   params [host]   one idg_params, copied during the call
  *   out    [device] nx*ny*nz fp32, receives I_n (n_iter = 0 copies cube)
@@ -246,6 +246,10 @@ int idg_wavelet_transform(const float *cube, int nx, int ny, int nz, int wavelet
  * bands") -- and transform back.  Pre-smoothing is a separate idg_gaussian_filter call.
  *   thresholds [host] `levels` floats >= 0, in units of rms;  rms > 0: noise level of the original cube
  *   cube, out as for idg_wavelet_transform.  Invalid wavelet, levels, thresholds or rms: IDG_ERR_PARAM.
+ * Le Gall 5/3: the default path fuses the three axes of a level and works out of place on compact lattices in a
+ * stream-ordered temporary of ~1.3 cubes (see idg_release_temporaries); when that cannot be allocated, or with
+ * IDG_OPT_KERNEL = 2 (1: two-phase passes), it runs the in-place passes, which need no memory ("does not require
+ * additional memory").  All paths give bit-identical results.
  */
 int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, int levels, const float *thresholds,
                        float rms, float *out, void *stream);
@@ -267,6 +271,16 @@ enum { IDG_OPT_KERNEL = 0, IDG_OPT_FUSE = 1, IDG_OPT_ZCHUNK = 2, IDG_OPT_TILE = 
        IDG_OPT_HOST_SLABS = 5, IDG_OPT_COUNT_ = 6 };
 int idg_set_option(int key, int value);
 int idg_get_option(int key);
+
+/*
+ * Stream-ordered temporaries (the scratch cube of idg_filter, the device buffers of idg_filter_host when none
+ * are passed, the kernel weights of a rotated Gaussian, the lattices of the Le Gall filter) come from a memory
+ * pool private to the library, one per device, which keeps the memory it has been given between calls so that
+ * a call does not pay the driver's map / unmap again.  idg_release_temporaries() returns everything that is not
+ * in use on the current device to the driver (synchronise the streams that used the library first).
+ * Returns IDG_OK or a cudaError_t.
+ */
+int idg_release_temporaries(void);
 
 /*
  * Number of kernel launches the last filter call on this thread enqueued

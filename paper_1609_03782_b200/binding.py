@@ -26,7 +26,7 @@ SYMBOLS = ("idg_version", "idg_status_string", "idg_params_check", "idg_workspac
            "idg_set_option", "idg_get_option", "idg_last_launch_count", "idg_last_plan",
            "idg_box_filter", "idg_gaussian_filter", "idg_gaussian_radii",
            "idg_mask_sums", "idg_cube_stats", "idg_quality", "idg_filter_pm",
-           "idg_wavelet_transform", "idg_wavelet_filter", "idg_histogram")
+           "idg_wavelet_transform", "idg_wavelet_filter", "idg_histogram", "idg_release_temporaries")
 WAVELET_HAAR, WAVELET_LEGALL53 = 0, 1
 
 
@@ -100,6 +100,8 @@ def lib() -> ctypes.CDLL:
         L.idg_get_option.restype = i
         L.idg_get_option.argtypes = [i]
         L.idg_last_launch_count.restype = i
+        L.idg_release_temporaries.restype = i
+        L.idg_release_temporaries.argtypes = []
         L.idg_last_plan.restype = ctypes.c_char_p
         f = ctypes.c_float
         L.idg_box_filter.restype = i
@@ -165,6 +167,11 @@ def idg_set_option(key: int, value: int) -> None:
 
 def idg_get_option(key: int) -> int:
     return int(lib().idg_get_option(key))
+
+
+def idg_release_temporaries() -> None:
+    """Hand the library's cached stream-ordered temporaries back to the driver (idg.h)."""
+    _check(lib().idg_release_temporaries())
 
 
 def idg_last_launch_count() -> int:

@@ -709,6 +709,8 @@ int idg_get_option(int key)
     return g_opt[key];
 }
 
+int idg_release_temporaries(void) { return (int)idg::temp_trim(); }
+
 int idg_last_launch_count(void) { return t_launches; }
 
 const char *idg_last_plan(void) { return t_plan; }

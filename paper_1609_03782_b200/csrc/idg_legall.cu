@@ -137,20 +137,30 @@ __device__ __forceinline__ void stage_tile(float *sm, const LArgs &A, const CUte
     }
 }
 
-// A complete row of the staged tile <-> registers, as ten 16-byte accesses.
-__device__ __forceinline__ void load_row(float (&v)[PX], const float *row)
+// A complete row of the staged tile <-> registers, as ten 16-byte accesses.  The row pitch is an even number of
+// 16-byte quads, so rows R and R + 4 start in the same bank group: threads whose row has bit 2 set touch the
+// quads of each pair in the opposite order (q ^ 1), which makes the eight lanes of a phase hit distinct banks.
+__device__ __forceinline__ void load_row(float (&v)[PX], const float *row, bool swap)
 {
 #pragma unroll
-    for (int q = 0; q < PX / 4; ++q) {
-        const float4 t = reinterpret_cast<const float4 *>(row)[q];
-        v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+    for (int q = 0; q < PX / 4; q += 2) {
+        const float4 a = reinterpret_cast<const float4 *>(row)[swap ? q + 1 : q];
+        const float4 b = reinterpret_cast<const float4 *>(row)[swap ? q : q + 1];
+        v[4 * q + 0] = swap ? b.x : a.x; v[4 * q + 1] = swap ? b.y : a.y;
+        v[4 * q + 2] = swap ? b.z : a.z; v[4 * q + 3] = swap ? b.w : a.w;
+        v[4 * q + 4] = swap ? a.x : b.x; v[4 * q + 5] = swap ? a.y : b.y;
+        v[4 * q + 6] = swap ? a.z : b.z; v[4 * q + 7] = swap ? a.w : b.w;
     }
 }
-__device__ __forceinline__ void store_row(float *row, const float (&v)[PX])
+__device__ __forceinline__ void store_row(float *row, const float (&v)[PX], bool swap)
 {
 #pragma unroll
-    for (int q = 0; q < PX / 4; ++q)
-        reinterpret_cast<float4 *>(row)[q] = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+    for (int q = 0; q < PX / 4; q += 2) {
+        const float4 lo = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+        const float4 hi = make_float4(v[4 * q + 4], v[4 * q + 5], v[4 * q + 6], v[4 * q + 7]);
+        reinterpret_cast<float4 *>(row)[swap ? q + 1 : q] = swap ? hi : lo;
+        reinterpret_cast<float4 *>(row)[swap ? q : q + 1] = swap ? lo : hi;
+    }
 }
 
 template <bool TMA>
@@ -163,9 +173,10 @@ __global__ void __launch_bounds__(FNT, 2) idg_legall_fwd_kernel(const __grid_con
     // x lines: one thread per (y, z) row of the staged tile
     for (int r = threadIdx.x; r < EY * EZ; r += FNT) {
         float v[PX];
-        load_row(v, sm + r * PX);
+        const bool swap = (r & 4) != 0;
+        load_row(v, sm + r * PX, swap);
         fwd_line<FX, XO - 2>(v, x0, A.mx);
-        store_row(sm + r * PX, v);
+        store_row(sm + r * PX, v, swap);
     }
     __syncthreads();
     // y lines: (interior x, every z)
@@ -220,8 +231,8 @@ __global__ void __launch_bounds__(FNT, 2) idg_legall_inv_kernel(const __grid_con
     const int x0 = blockIdx.x * FX, y0 = blockIdx.y * FY, z0 = blockIdx.z * FZ;
     stage_tile<TMA>(sm, A, &map, x0 - XO, y0 - 1, z0 - 1);
     // z lines: hard thresholds by band as the column is read (reading W3), then the inverse lifting
-    for (int p = threadIdx.x; p < EX * EY; p += FNT) {
-        const int lx = XO - 1 + p % EX, ly = p / EX;      // staged columns x0 - 1 .. x0 + 33
+    for (int p = threadIdx.x; p < PX * EY; p += FNT) {      // every staged column: a warp never straddles rows
+        const int lx = p % PX, ly = p / PX;
         const bool even_xy = (((x0 - XO + lx) | (y0 - 1 + ly)) & 1) == 0;
         float *col = sm + ly * PX + lx;
         float v[EZ];
@@ -237,9 +248,11 @@ __global__ void __launch_bounds__(FNT, 2) idg_legall_inv_kernel(const __grid_con
     }
     __syncthreads();
     // y lines: (every x, interior z)
-    for (int t = threadIdx.x; t < EX * FZ; t += FNT) {
+    // (columns 0 .. 31 of a plane by one warp, then columns 32 .. 39 of four planes: conflict-free both ways)
+    for (int t = threadIdx.x; t < PX * FZ; t += FNT) {
         float v[EY];
-        float *col = sm + (1 + t / EX) * PP + XO - 1 + (t % EX);
+        const int lx = t < 32 * FZ ? t % 32 : 32 + t % 8, lz = t < 32 * FZ ? t / 32 : (t - 32 * FZ) / 8;
+        float *col = sm + (1 + lz) * PP + lx;
 #pragma unroll
         for (int l = 0; l < EY; ++l) v[l] = col[l * PX];
         inv_line<FY, 0>(v, y0, A.my);
@@ -250,10 +263,12 @@ __global__ void __launch_bounds__(FNT, 2) idg_legall_inv_kernel(const __grid_con
     // x lines: (interior y, interior z)
     for (int r = threadIdx.x; r < FY * FZ; r += FNT) {
         float v[PX];
-        float *row = sm + (1 + r / FY) * PP + (1 + r % FY) * PX;
-        load_row(v, row);
+        const int R = (1 + r / FY) * EY + 1 + r % FY;      // row index in the staged tile
+        float *row = sm + R * PX;
+        const bool swap = (R & 4) != 0;
+        load_row(v, row, swap);
         inv_line<FX, XO - 1>(v, x0, A.mx);
-        store_row(row, v);
+        store_row(row, v, swap);
     }
     __syncthreads();
     // coalesced write of the interior: dense (16-byte stores when the rows allow), or onto the all-even
@@ -261,16 +276,16 @@ __global__ void __launch_bounds__(FNT, 2) idg_legall_inv_kernel(const __grid_con
     const long long oplane = (long long)A.ox * A.oy;
     if (A.os == 1 && (A.ox & 3) == 0 && ((uintptr_t)A.full & 15u) == 0) {
         const int q = threadIdx.x % (FX / 4), gx = x0 + 4 * q;            // ox % 4 == 0: a quad is inside or outside
+        const int nzv = min(FZ, A.mz - z0), nyv = min(FY, A.my - y0);
         if (gx < A.mx) {
-            for (int ly = threadIdx.x / (FX / 4); ly < FY; ly += FNT / (FX / 4)) {
-                const int gy = y0 + ly;
-                if (gy >= A.my) break;
-                float *o = A.full + (long long)gy * A.ox + gx + (long long)z0 * oplane;
-                const float *s = sm + PP + (1 + ly) * PX + XO + 4 * q;
-                const int nzv = min(FZ, A.mz - z0);
-#pragma unroll 8
-                for (int lz = 0; lz < nzv; ++lz)
-                    *reinterpret_cast<float4 *>(o + lz * oplane) = *reinterpret_cast<const float4 *>(s + lz * PP);
+            float *o = A.full + (long long)y0 * A.ox + gx + (long long)z0 * oplane;
+            const float *s = sm + PP + PX + XO + 4 * q;
+#pragma unroll 4
+            for (int r = threadIdx.x / (FX / 4); r < FY * FZ; r += FNT / (FX / 4)) {       // r = (lz, ly)
+                const int ly = r % FY, lz = r / FY;
+                if (ly < nyv && lz < nzv)
+                    *reinterpret_cast<float4 *>(o + lz * oplane + (long long)ly * A.ox) =
+                        *reinterpret_cast<const float4 *>(s + lz * PP + ly * PX);
             }
         }
     } else {

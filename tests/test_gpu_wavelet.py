@@ -170,3 +170,16 @@ def test_argument_errors(B):
     assert e.value.status == -4
     with pytest.raises(TypeError):
         B.idg_wavelet_transform(a.cpu(), 0, 1)
+
+
+def test_release_temporaries(B):
+    """The private pool keeps the Le Gall temporaries (~1.3 cubes) between calls; idg_release_temporaries
+    hands them back to the driver, and the next call simply allocates again."""
+    a = torch.from_numpy(noisy((96, 128, 256), 5)).cuda()              # 12.6 MB cube -> ~16 MB of temporaries
+    ref = B.idg_wavelet_filter(a, B.WAVELET_LEGALL53, (1.0, 1.4, 1.7))
+    torch.cuda.synchronize()
+    held = torch.cuda.mem_get_info()[0]
+    B.idg_release_temporaries()
+    freed = torch.cuda.mem_get_info()[0]
+    assert freed >= held + 8 * 2 ** 20
+    assert torch.equal(B.idg_wavelet_filter(a, B.WAVELET_LEGALL53, (1.0, 1.4, 1.7)), ref)
