@@ -30,7 +30,7 @@ namespace idg {
 namespace {
 
 constexpr int FX = 32, FY = 16, FZ = 32;                    // interior tile, lattice samples (all even)
-constexpr int EX = FX + 3, EY = FY + 3, EZ = FZ + 3;        // with the lifting halo
+constexpr int EY = FY + 3, EZ = FZ + 3;                     // with the lifting halo (x: see PX)
 constexpr int PX = 40, XO = 4;                              // staged row: samples x0 - XO .. x0 - XO + PX - 1
 constexpr int PP = PX * EY;                                 // plane pitch
 constexpr int FNT = 256;

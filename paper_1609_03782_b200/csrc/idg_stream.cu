@@ -294,7 +294,7 @@ __device__ __forceinline__ void run(const Launch &L, const StreamArgs &A, const 
         for (int i = 0; i < NS - 2; ++i) issue_ahead<TL, Y>(L, A, M, cur, i, (P.s + i) % NS, sbase);
     }
 
-    Seg S;
+    Seg S = {};      // filled by segment_setup before the first plane job
     unsigned seg = 0;
     F4 ring[3][TR][R];
 #pragma unroll
