@@ -109,13 +109,12 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
             if (!fuse) fuse = 2;
             if (!tile) tile = 2;
         } else if (can_tma) {
+            // four fused iterations per launch, one 8-warp CTA per SM: a quarter of the DRAM traffic of an
+            // un-fused sweep; with the 10-operation update this beats two iterations on two CTAs per SM at every
+            // size measured (profiles/r1g_notes.md).  The tail of n_iter mod 4 iterations runs as one launch of
+            // the kernel built for that depth (below).
             kernel = 3;
-            if (work >= 1.6e7) {
-                if (!fuse) fuse = 2;
-                if (!tile) tile = 2;
-            } else if (!fuse) {
-                fuse = 3;
-            }
+            if (!fuse) fuse = 4;
         } else {
             kernel = can_tile ? 2 : 1;
         }
@@ -135,8 +134,6 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     } else {
         fuse = 1;
     }
-    if (kernel == 3 && tile > 2) tile = 0;
-    if (kernel == 3 && fuse > 2 && tile == 2) tile = 1;
     {
         static const char *const names[5] = {"", "idg_naive_kernel", "idg_tiled_kernel", "idg_tma_kernel",
                                              "idg_stream_kernel"};
@@ -192,8 +189,17 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     }
     for (int done = 0; done < max_n; done += fuse) {
         L.iter_done = done;
+        int tile_now = tile;
+        if (kernel == 3) {
+            // the last launch applies the remaining r < fuse iterations: give it the kernel built for depth r
+            // (route() sees remaining <= r for every cube, so it is that cube's last launch either way)
+            const int rem = max_n - done;
+            L.fuse = rem < fuse ? rem : fuse;
+            if (tile_now == 0) tile_now = L.fuse <= 2 ? 2 : (L.fuse == 3 ? 3 : 1);
+            else if (L.fuse <= 2 && tile_now > 2) tile_now = 0;
+        }
         e = (kernel == 4)   ? idg::launch_stream(L, g_opt[IDG_OPT_CTAS], tile, st)
-            : (kernel == 3) ? idg::launch_tma(L, g_opt[IDG_OPT_ZCHUNK], tile, st)
+            : (kernel == 3) ? idg::launch_tma(L, g_opt[IDG_OPT_ZCHUNK], tile_now, st)
             : (kernel == 2) ? idg::launch_tiled(L, g_opt[IDG_OPT_ZCHUNK], st)
                             : idg::launch_naive(L, st);
         if (e != cudaSuccess) return (int)e;

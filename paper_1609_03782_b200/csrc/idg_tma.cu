@@ -371,16 +371,25 @@ bool tma_supported(int nx, int ny, int nz, const void *in, const void *out, cons
     return tmap_available();
 }
 
-// tile: 0 auto | 1 = 128x64 tile, 512 threads, one CTA per SM | 2 = 128x32 tile, 256 threads,
-// two CTAs per SM (T <= 2; deeper fusion needs the registers of a lone CTA)
+// tile (T = fused iterations): T <= 2: 0, 1 = 128x64 tile, 512 threads, one CTA per SM | 2 = 128x32 tile, 256
+// threads, two CTAs per SM.  T >= 3 needs the registers of a lone CTA: 0, 1 = 128x32 tile, 256 threads | 3 =
+// 128x48 / 128x36 tile, 384 threads (T = 3: strips of 4 rows; T = 4: strips of 3).
 cudaError_t launch_tma(const Launch &L, int zchunk, int tile, cudaStream_t st)
 {
     const bool small = (tile == 2);
     switch (L.fuse) {
     case 1: return small ? launch_cfg<1, 4, 8, 4, 2>(L, zchunk, st) : launch_cfg<1, 4, 16, 4, 1>(L, zchunk, st);
     case 2: return small ? launch_cfg<2, 4, 8, 4, 2>(L, zchunk, st) : launch_cfg<2, 4, 16, 4, 1>(L, zchunk, st);
-    case 3: return launch_cfg<3, 4, 8, 4, 1>(L, zchunk, st);
-    case 4: return launch_cfg<4, 4, 8, 4, 1>(L, zchunk, st);
+    case 3:
+        switch (tile) {
+        case 3: return launch_cfg<3, 4, 12, 4, 1>(L, zchunk, st);
+        default: return launch_cfg<3, 4, 8, 4, 1>(L, zchunk, st);
+        }
+    case 4:
+        switch (tile) {
+        case 3: return launch_cfg<4, 3, 12, 4, 1>(L, zchunk, st);
+        default: return launch_cfg<4, 4, 8, 4, 1>(L, zchunk, st);
+        }
     default: return cudaErrorInvalidValue;
     }
 }

@@ -96,11 +96,12 @@ def test_zchunk_variants(B, oracle, kernel, fuse, zchunk):
     assert err(gpu(B, a, 7, p), ref, 2.0) <= TOL
 
 
-@pytest.mark.parametrize("tile", [1, 2])
-@pytest.mark.parametrize("fuse", [1, 2, 4])
+@pytest.mark.parametrize("tile", [1, 2, 3])
+@pytest.mark.parametrize("fuse", [1, 2, 3, 4])
 def test_tma_tile_variants(B, oracle, fuse, tile):
-    """Both tilings of the TMA kernel (128x64 one CTA/SM, 128x32 two CTAs/SM) on a cube spanning
-    several tiles in x and y with ragged tails, and on the config-0 cube."""
+    """The tilings of the TMA kernel (T <= 2: 128x64 one CTA/SM, 128x32 two CTAs/SM; T >= 3: 8 or 12 warps
+    of one CTA/SM) on a cube spanning several tiles in x and y with ragged tails, and on the config-0
+    cube; n = 6 and 10 also exercise the tail launch of n mod T iterations."""
     from paper_1609_03782_b200 import synth
     set_plan(B, (3, fuse), 0, tile)
     rng = np.random.default_rng(17)
@@ -391,7 +392,7 @@ def test_fused_kernels_are_bitwise_equal_to_the_naive_kernel_and_repeatable(B, p
     p = B.Params(K=1.5, tau=0.03, cx=5.0, cy=4.0, cz=6.0, rms=1.0)
     set_plan(B, (1, 0))
     ref = B.idg_filter(x, 7, p)
-    for tile in ((1, 2) if plan[0] >= 3 and plan[1] <= 2 else (0,)):
+    for tile in ((1, 2) if plan[0] >= 3 and plan[1] <= 2 else ((0, 3) if plan[0] == 3 else (0,))):
         for rep in range(4):
             set_plan(B, plan, 0, tile)
             out = B.idg_filter(x, 7, p)
