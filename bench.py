@@ -377,7 +377,7 @@ def run_ours(args) -> None:
         lane_ops = 10.0 * value * 1e9 / 1e12                       # 10 FP32 lane-ops per voxel-iteration
         peak_ops = 148 * 128 * 1.965e9 / 1e12
         line["roofline"]["alu"] = {"achieved": lane_ops, "peak": peak_ops, "unit": "T lane-op/s", "frac": lane_ops / peak_ops,
-                                   "note": "useful voxel-iterations only; halo recomputation (x 1.3-1.4) comes on top"}
+                                   "note": "useful voxel-iterations only; halo recomputation (x 1.2 at T = 2 to x 1.45 at T = 4) comes on top"}
     if filt is not None and filt[0] == "gauss" and any(filt[2]):     # rotated Gaussian: bound by FP32, not by HBM
         r = B.idg_gaussian_radii(filt[1], filt[2])[0]
         flops = 2.0 * (2 * r + 1) ** 3 * N
