@@ -76,7 +76,7 @@ def ncu_traffic_bytes(kernel_tag: str):
     p = os.path.join(ROOT, "profiles", "traffic.txt")
     try:
         for line in open(p):
-            k, _, v = line.partition("=")
+            k, _, v = line.partition(" = ")              # the key itself holds '=' signs ("fuse=4")
             if k.strip() == kernel_tag:
                 return float(v.split()[0])
     except Exception:

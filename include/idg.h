@@ -132,7 +132,7 @@ int idg_filter_batched(const float *cubes, int nx, int ny, int nz, int batch,
  * End-to-end convenience for HOST buffers (the paper's T_p includes the
  * transfers): copies cube_host to the device, filters, copies
  * I_n to out_host and synchronises `stream` before returning.  Cubes of 64 MB
- * and more are cut into up to 8 z slabs (each filtered with n_iter halo planes
+ * and more are cut into up to 16 z slabs (each filtered with n_iter halo planes
  * per side, bit-identical results) so that upload, filtering and download
  * overlap on two internal copy streams; pinned host memory is needed for that.
  *   cube_host, out_host [host] nx*ny*nz fp32 (pinned memory gives full PCIe rate)
@@ -264,7 +264,7 @@ int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, i
  *   IDG_OPT_TILE     0 auto | 1 = 128x64 tile, one 512-thread CTA per SM | 2 = 128x32 tile, two
  *                    256-thread CTAs per SM | 3, 4 = further tilings of kernel 4 (see idg_stream.cu)
  *   IDG_OPT_CTAS     0 auto | >0  = persistent grid size of kernel 4
- *   IDG_OPT_HOST_SLABS  0 auto | 1..8 = z slabs of the idg_filter_host transfer/compute pipeline (1 = one piece)
+ *   IDG_OPT_HOST_SLABS  0 auto | 1..16 = z slabs of the idg_filter_host transfer/compute pipeline (1 = one piece)
  * idg_get_option returns the current value, or IDG_ERR_OPTION.
  */
 enum { IDG_OPT_KERNEL = 0, IDG_OPT_FUSE = 1, IDG_OPT_ZCHUNK = 2, IDG_OPT_TILE = 3, IDG_OPT_CTAS = 4,

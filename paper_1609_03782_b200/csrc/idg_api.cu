@@ -287,6 +287,8 @@ int idg_filter(const float *cube, int nx, int ny, int nz, int n_iter, const idg_
     return e == cudaSuccess ? IDG_OK : (int)e;
 }
 
+constexpr int kMaxSlabs = 16;      // z slabs of the idg_filter_host pipeline
+
 int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
                     const idg_params *params, float *out_host, void *dev_buffers,
                     size_t dev_buffers_bytes, void *stream)
@@ -324,12 +326,15 @@ int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
     if (slabs == 0) {
         slabs = 1;
         if (bytes >= (64u << 20) && n_iter > 0) {
-            const int thick = 3 * n_iter > 16 ? 3 * n_iter : 16;       // keep the halo overhead below ~70 %
+            // thin slabs shorten the pipeline's tail (the last slab's filtering and download); their 2 n halo planes
+            // are recomputed, which the GPU has time for: it idles on the PCIe link
+            const int thick = 3 * n_iter / 2 > 16 ? 3 * n_iter / 2 : 16;
             slabs = nz / thick;
-            if (slabs > 8) slabs = 8;
+            if (slabs > kMaxSlabs) slabs = kMaxSlabs;
             if (slabs < 1) slabs = 1;
         }
     }
+    if (slabs > kMaxSlabs) slabs = kMaxSlabs;
     if (slabs > nz) slabs = nz;
     const size_t plane_b = (size_t)nx * ny * sizeof(float);
     const int zs = (nz + slabs - 1) / slabs;
@@ -338,12 +343,12 @@ int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
     const size_t slab_ws = idg_workspace_bytes(nx, ny, max_planes, 1);
     if (slabs > 1 && n_iter > 0 && 2 * slab_al + slab_ws <= need - cube_al) {
         static cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
-        static cudaEvent_t ev_h[8], ev_c[8], ev_d[8], ev_begin;
+        static cudaEvent_t ev_h[kMaxSlabs], ev_c[kMaxSlabs], ev_d[kMaxSlabs], ev_begin;
         static bool ready = false;
         if (!ready) {
             e = cudaStreamCreateWithFlags(&s_h2d, cudaStreamNonBlocking);
             if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s_d2h, cudaStreamNonBlocking);
-            for (int i = 0; i < 8 && e == cudaSuccess; ++i) {
+            for (int i = 0; i < kMaxSlabs && e == cudaSuccess; ++i) {
                 e = cudaEventCreateWithFlags(&ev_h[i], cudaEventDisableTiming);
                 if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_c[i], cudaEventDisableTiming);
                 if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_d[i], cudaEventDisableTiming);
@@ -704,7 +709,7 @@ int idg_set_option(int key, int value)
     if (key == IDG_OPT_ZCHUNK && value < 0) return IDG_ERR_OPTION;
     if (key == IDG_OPT_TILE && (value < 0 || value > 4)) return IDG_ERR_OPTION;
     if (key == IDG_OPT_CTAS && value < 0) return IDG_ERR_OPTION;
-    if (key == IDG_OPT_HOST_SLABS && (value < 0 || value > 8)) return IDG_ERR_OPTION;
+    if (key == IDG_OPT_HOST_SLABS && (value < 0 || value > kMaxSlabs)) return IDG_ERR_OPTION;
     g_opt[key] = value;
     return IDG_OK;
 }

@@ -68,3 +68,13 @@ def test_reference_arm_under_torchrun_world2():
     assert r["impl"] == "reference" and r["n_gpus"] == 2 and r["unit"] == "Gvoxel-iter/s"
     assert r["cpu_baseline"]["kind"] == "oracle" and r["cpu_baseline"]["value"] == r["value"] > 0
     assert r["e2e"] == {"value": r["value"], "unit": r["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+
+
+def test_traffic_table_lookup():
+    """bench.py's `roofline.traffic` comes from profiles/traffic.txt, keyed by "<plan> <workload>"; the plan
+    string itself contains '=' signs."""
+    sys.path.insert(0, ROOT)
+    import bench
+    v = bench.ncu_traffic_bytes("idg_tma_kernel fuse=4 tile=0 cfg3_1024x1024x512_n20")
+    assert v is not None and 4.2e9 < v < 4.6e9          # one read + one write of the 2.147 GB cube, plus halo
+    assert bench.ncu_traffic_bytes("no such kernel cfg3_1024x1024x512_n20") is None

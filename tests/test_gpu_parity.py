@@ -327,7 +327,7 @@ def test_host_entry_point(B, oracle):
     assert torch.equal(out, out2)
 
 
-@pytest.mark.parametrize("slabs", [2, 3, 8])
+@pytest.mark.parametrize("slabs", [2, 3, 8, 16])
 def test_host_entry_point_slab_pipeline(B, oracle, slabs):
     """idg_filter_host cut into z slabs (upload / filter / download overlapped): every slab is filtered with
     n halo planes per side, so the result is bit-identical to the one-piece call (domain of dependence, P8);
