@@ -204,7 +204,7 @@ __global__ void __launch_bounds__(NT) idg_lift_strip_kernel(const __grid_constan
 
 // ---- Haar thresholding filter, up to 3 levels, in ONE pass ------------------------------------------------
 // A Haar pair never leaves its 2-block, so the whole L-level transform of an 8 x 8 x 8 aligned block depends on
-// that block only.  A CTA stages a 32 x 8 x 8 region in shared memory, runs forward levels 1..L (a thread per
+// that block only.  A CTA stages a 64 x 8 x 8 region in shared memory, runs forward levels 1..L (a thread per
 // 2 x 2 x 2 lattice block: its four x pairs, then y pairs, then z pairs -- the same operations in the same order
 // as the per-axis passes), thresholds, runs the inverse levels L..1 and writes the region back: the cube is read
 // once and written once (8 B per voxel) instead of ~19 in-place passes.  Safe in place (out == cube).
@@ -215,7 +215,7 @@ struct HArgs {
     float thr[3];
 };
 
-constexpr int HX = 32, HY = 8, HZ = 8, HPAD = 33;            // region and padded row length (bank conflicts)
+constexpr int HX = 64, HY = 8, HZ = 8, HPAD = 65;            // region and padded row length (bank conflicts)
 
 template <bool INV>
 __device__ __forceinline__ void haar_pair(float &e, float &o)
