@@ -95,26 +95,16 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     int fuse = g_opt[IDG_OPT_FUSE];
     int tile = g_opt[IDG_OPT_TILE];
     if (kernel == 0) {
-        // Measured on B200 (profiles/): batches and cubes of at most 128 columns run best on the persistent
-        // kernel (one tile column, no idle tail between cubes); large single cubes on the z-chunked TMA
-        // kernel with two CTAs per SM; cubes too small to fill the GPU want few, deeply fused launches.
+        // Measured on B200 (profiles/r1g_notes.md, r1h_notes.md): the z-chunked TMA kernel everywhere it applies.
+        // Four fused iterations per launch (one 8-warp CTA per SM) move a quarter of the DRAM bytes of an un-fused
+        // sweep and need the fewest launches; only when the GPU is full AND the cubes are thin in z do the 2 T
+        // warm-up planes per z chunk and the taller halo cost more than that saves: then two iterations on two
+        // CTAs per SM.  The tail of n_iter mod T iterations runs as one launch of the kernel built for that depth.
+        // Cubes of at most 128 columns (the interactive batches) use the single-tile-column variant.
         const double work = (double)N * (double)batch;
-        // the persistent kernel pays ~2T + 3 warm-up planes per CTA: it wants >= 24 planes per team
-        // (two 128x32-tile CTAs per SM; x tiles of 30 float4 + one halo column each)
-        const int nx4 = nx / 4, tiles_x = nx4 <= 2 ? 1 : (nx4 - 2 + 29) / 30, tiles_y = (ny + 27) / 28;
-        const double teams = (double)(296 / (tiles_x < 296 ? tiles_x : 296));
-        const double planes_per_team = (double)batch * tiles_y * (double)nz / (teams < 1.0 ? 1.0 : teams);
-        if (can_stream && (batch > 1 || nx <= 128) && planes_per_team >= 24.0) {
-            kernel = 4;
-            if (!fuse) fuse = 2;
-            if (!tile) tile = 2;
-        } else if (can_tma) {
-            // four fused iterations per launch, one 8-warp CTA per SM: a quarter of the DRAM traffic of an
-            // un-fused sweep; with the 10-operation update this beats two iterations on two CTAs per SM at every
-            // size measured (profiles/r1g_notes.md).  The tail of n_iter mod 4 iterations runs as one launch of
-            // the kernel built for that depth (below).
+        if (can_tma) {
             kernel = 3;
-            if (!fuse) fuse = 4;
+            if (!fuse) fuse = (nz < 100 && work >= 4.0e6) ? 2 : 4;
         } else {
             kernel = can_tile ? 2 : 1;
         }

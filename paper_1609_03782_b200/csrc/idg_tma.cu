@@ -119,7 +119,9 @@ struct Smem {
     static constexpr size_t kBytes = kBarOff + NS * sizeof(uint64_t);
 };
 
-template <int TL, int R, int WARPS, int NS, int TMAX>
+// ONE: the cube has at most 128 columns, so a single tile column covers a row with all 32 lanes valid and no halo
+// lanes; the x faces are replicated by patching the shuffled neighbour of the first / last float4 of the row.
+template <int TL, int R, int WARPS, int NS, int TMAX, bool ONE>
 __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restrict__ dst, const Launch &L,
                                          const TmaArgs &A, const CubeParams &prm, int b,
                                          unsigned char *smem)
@@ -135,9 +137,10 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
     const int nx4 = L.nx >> 2;
     const int vy = TILE_Y - 2 * A.halo;
     const int ti = blockIdx.x % A.tiles_x, tj = blockIdx.x / A.tiles_x;
-    const int tx0 = (ti * kValidLanes - 1) * 4;          // cube x of tile column 0
+    const int tx0 = ONE ? 0 : (ti * kValidLanes - 1) * 4;   // cube x of tile column 0
     const int ty0 = tj * vy - A.halo;                    // cube y of tile row 0
-    const int x4 = ti * kValidLanes - 1 + lane;
+    const int x4 = ONE ? lane : ti * kValidLanes - 1 + lane;
+    const bool x_first = ONE && lane == 0, x_last = ONE && lane == nx4 - 1;
     const int row0 = wy * R;
     const int z0 = blockIdx.y * A.zchunk;
     const int z1 = min(z0 + A.zchunk, L.nz);
@@ -148,9 +151,11 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
     unsigned ok = 0, fix = 0;
     bool rev = false;
     int slane = lane;
-    if (x4 < 0) { slane = lane + (-1 - x4) - x4; rev = true; }                 // x4' = -1 - x4
-    else if (x4 >= nx4) { slane = lane + (2 * nx4 - 1 - x4) - x4; rev = true; }
-    if (slane < 0 || slane >= kLanes) { slane = lane; rev = false; }            // beyond one reflection: unused cell
+    if (!ONE) {
+        if (x4 < 0) { slane = lane + (-1 - x4) - x4; rev = true; }             // x4' = -1 - x4
+        else if (x4 >= nx4) { slane = lane + (2 * nx4 - 1 - x4) - x4; rev = true; }
+        if (slane < 0 || slane >= kLanes) { slane = lane; rev = false; }        // beyond one reflection: unused cell
+    }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int row = row0 + r, gy = ty0 + row;
@@ -161,7 +166,7 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
         if (srow < 0 || srow >= TILE_Y) srow = row;
         scell[r] = srow * kTileX + slane * 4;
         if (scell[r] != cell[r]) fix |= 1u << r;
-        if (lane >= 1 && lane <= kValidLanes && x4 < nx4 && row >= A.halo && row < TILE_Y - A.halo &&
+        if ((ONE || (lane >= 1 && lane <= kValidLanes)) && x4 < nx4 && row >= A.halo && row < TILE_Y - A.halo &&
             gy < L.ny)
             ok |= 1u << r;
     }
@@ -250,8 +255,12 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 const F4 &c = cc[t][r];
-                const float left = __shfl_up_sync(0xffffffffu, c.w, 1);
-                const float right = __shfl_down_sync(0xffffffffu, c.x, 1);
+                float left = __shfl_up_sync(0xffffffffu, c.w, 1);
+                float right = __shfl_down_sync(0xffffffffu, c.x, 1);
+                if (ONE) {
+                    left = x_first ? c.x : left;                  // zero-flux faces (reading R1)
+                    right = x_last ? c.w : right;
+                }
                 const F4 &ym = (r == 0) ? up : cc[t][r - 1];
                 const F4 &yp = (r == R - 1) ? dn : cc[t][r + 1];
                 const F4 o = update4(c, left, right, ym, yp, zm[t][r], nw[t][r], kc);
@@ -284,7 +293,7 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
     }
 }
 
-template <int T, int R, int WARPS, int NS, int MINB>
+template <int T, int R, int WARPS, int NS, int MINB, bool ONE>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 idg_tma_kernel(const __grid_constant__ Launch L, const __grid_constant__ TmaArgs A,
                const __grid_constant__ Maps M)
@@ -298,10 +307,10 @@ idg_tma_kernel(const __grid_constant__ Launch L, const __grid_constant__ TmaArgs
     if (now == 0) return;
     const size_t off = (size_t)b * (size_t)L.nx * (size_t)L.ny * (size_t)L.nz;
     const CUtensorMap *map = (src == L.scratch + off) ? &M.scratch : (src == L.out + off) ? &M.out : &M.in;
-    if (now == T) tma_body<T, R, WARPS, NS, T>(map, dst, L, A, prm, b, smem);
-    else if (T > 1 && now == 1) tma_body<1, R, WARPS, NS, T>(map, dst, L, A, prm, b, smem);
-    else if (T > 2 && now == 2) tma_body<(T > 2 ? 2 : 1), R, WARPS, NS, T>(map, dst, L, A, prm, b, smem);
-    else if (T > 3 && now == 3) tma_body<(T > 3 ? 3 : 1), R, WARPS, NS, T>(map, dst, L, A, prm, b, smem);
+    if (now == T) tma_body<T, R, WARPS, NS, T, ONE>(map, dst, L, A, prm, b, smem);
+    else if (T > 1 && now == 1) tma_body<1, R, WARPS, NS, T, ONE>(map, dst, L, A, prm, b, smem);
+    else if (T > 2 && now == 2) tma_body<(T > 2 ? 2 : 1), R, WARPS, NS, T, ONE>(map, dst, L, A, prm, b, smem);
+    else if (T > 3 && now == 3) tma_body<(T > 3 ? 3 : 1), R, WARPS, NS, T, ONE>(map, dst, L, A, prm, b, smem);
 }
 
 bool encode_map(CUtensorMap *m, const float *base, const Launch &L, int tile_y)
@@ -336,7 +345,8 @@ cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st)
     static_assert(S::kBytes * MINB <= 227 * 1024, "shared memory budget");
     TmaArgs A;
     A.halo = T;
-    A.tiles_x = (L.nx / 4 + kValidLanes - 1) / kValidLanes;
+    const bool one = L.nx <= kTileX;                     // a single tile column: no halo lanes
+    A.tiles_x = one ? 1 : (L.nx / 4 + kValidLanes - 1) / kValidLanes;
     A.tiles_y = (L.ny + (TILE_Y - 2 * T) - 1) / (TILE_Y - 2 * T);
     const long tiles = (long)A.tiles_x * A.tiles_y;
     if (tiles > 0x7fffffffL) return cudaErrorInvalidValue;
@@ -346,12 +356,12 @@ cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st)
     if (!encode_map(&M.in, L.in, L, TILE_Y) || !encode_map(&M.out, L.out, L, TILE_Y) ||
         !encode_map(&M.scratch, L.scratch, L, TILE_Y))
         return cudaErrorNotSupported;
-    auto kern = idg_tma_kernel<T, R, WARPS, NS, MINB>;
-    static bool attr_done = false;
-    if (!attr_done) {
+    auto kern = one ? idg_tma_kernel<T, R, WARPS, NS, MINB, true> : idg_tma_kernel<T, R, WARPS, NS, MINB, false>;
+    static bool attr_done[2] = {false, false};
+    if (!attr_done[one]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::kBytes);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        attr_done[one] = true;
     }
     dim3 grid((unsigned)tiles, (unsigned)((L.nz + A.zchunk - 1) / A.zchunk), (unsigned)L.batch);
     kern<<<grid, WARPS * 32, S::kBytes, st>>>(L, A, M);
