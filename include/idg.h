@@ -256,13 +256,15 @@ int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, i
 
 /*
  * Process-wide tuning knobs (tests and benchmarks; defaults give the fastest plan).
- *   IDG_OPT_KERNEL   0 auto | 1 naive (one thread per voxel) | 2 tiled z-streaming kernel (global loads)
- *                    | 3 tiled z-streaming kernel fed by TMA | 4 persistent warp-decoupled TMA kernel
- *                    (the fast path)
- *   IDG_OPT_FUSE     0 auto | 1..4 = diffusion iterations fused per launch (tiled kernels)
- *   IDG_OPT_ZCHUNK   0 auto | >0  = planes per CTA along z (tiled kernels)
- *   IDG_OPT_TILE     0 auto | 1 = 128x64 tile, one 512-thread CTA per SM | 2 = 128x32 tile, two
- *                    256-thread CTAs per SM | 3, 4 = further tilings of kernel 4 (see idg_stream.cu)
+ *   IDG_OPT_KERNEL   0 auto (kernel 3 wherever nx % 4 == 0 and the buffers are 16-byte aligned) | 1 naive (one
+ *                    thread per voxel) | 2 tiled z-streaming kernel (global loads) | 3 tiled z-streaming kernel
+ *                    fed by TMA (the fast path) | 4 persistent warp-decoupled TMA kernel
+ *   IDG_OPT_FUSE     0 auto (4, or 2 for full-GPU workloads of cubes thinner than 100 planes) | 1..4 = diffusion
+ *                    iterations fused per launch (kernels 2-4)
+ *   IDG_OPT_ZCHUNK   0 auto | >0  = planes per CTA along z (kernels 2, 3)
+ *   IDG_OPT_TILE     0 auto | kernel 3: 1 = one CTA per SM (T <= 2: 128x64 tile, 512 threads; T >= 3: 128x32
+ *                    tile, 256 threads), 2 = 128x32 tile, two 256-thread CTAs per SM (T <= 2), 3 = 384-thread CTA
+ *                    (T >= 3) | kernel 4: 1..4, see idg_stream.cu
  *   IDG_OPT_CTAS     0 auto | >0  = persistent grid size of kernel 4
  *   IDG_OPT_HOST_SLABS  0 auto | 1..16 = z slabs of the idg_filter_host transfer/compute pipeline (1 = one piece)
  * idg_get_option returns the current value, or IDG_ERR_OPTION.
