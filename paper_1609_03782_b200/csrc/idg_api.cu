@@ -408,6 +408,23 @@ static int ref_args(const float *cube, int nx, int ny, int nz, const float *out,
     return IDG_OK;
 }
 
+// Separable filter: the TMA-fed kernel where it applies (radii <= 4, nx % 4 == 0, 16-byte aligned; option kernel = 1
+// forces the general kernel), else idg_sep3d_kernel.  Returns the kernel name through `name`.
+static cudaError_t run_sep3d(const float *cube, float *out, int nx, int ny, int nz, const int r[3], const float *wx,
+                             const float *wy, const float *wz, cudaStream_t st, const char **name)
+{
+    *name = "idg_sep3d_kernel";
+    if (g_opt[IDG_OPT_KERNEL] != 1 && idg::sep3d_tma_supported(nx, ny, nz, r[0], r[1], r[2], cube, out)) {
+        const cudaError_t e = idg::launch_sep3d_tma(cube, out, nx, ny, nz, r[0], r[1], r[2], wx, wy, wz,
+                                                    g_opt[IDG_OPT_ZCHUNK], g_opt[IDG_OPT_TILE], st);
+        if (e != cudaErrorNotSupported) {
+            *name = "idg_sep3d_tma_kernel";
+            return e;
+        }
+    }
+    return idg::launch_sep3d(cube, out, nx, ny, nz, r[0], r[1], r[2], wx, wy, wz, st);
+}
+
 int idg_box_filter(const float *cube, int nx, int ny, int nz, int wx, int wy, int wz, float *out, void *stream)
 {
     t_launches = 0;
@@ -420,11 +437,12 @@ int idg_box_filter(const float *cube, int nx, int ny, int nz, int wx, int wy, in
         if (w[a] < 1 || !(w[a] & 1) || w[a] > 2 * idg::kSepMaxRadius + 1) return IDG_ERR_PARAM;
         for (int i = 0; i < w[a]; ++i) wt[a][i] = (float)(1.0 / (double)w[a]);     // PAPER.md:123, the mean
     }
-    const cudaError_t e = idg::launch_sep3d(cube, out, nx, ny, nz, wx / 2, wy / 2, wz / 2, wt[0], wt[1], wt[2],
-                                            (cudaStream_t)stream);
+    const int r[3] = {wx / 2, wy / 2, wz / 2};
+    const char *name;
+    const cudaError_t e = run_sep3d(cube, out, nx, ny, nz, r, wt[0], wt[1], wt[2], (cudaStream_t)stream, &name);
     if (e != cudaSuccess) return (int)e;
     t_launches = 1;
-    snprintf(t_plan, sizeof(t_plan), "idg_sep3d_kernel box %dx%dx%d", wx, wy, wz);
+    snprintf(t_plan, sizeof(t_plan), "%s box %dx%dx%d", name, wx, wy, wz);
     return IDG_OK;
 }
 
@@ -482,10 +500,11 @@ int idg_gaussian_filter(const float *cube, int nx, int ny, int nz, float fwhm_x,
             }
             for (int i = 0; i <= 2 * r[a]; ++i) wt[a][i] = (float)(g[i] / sum);
         }
-        const cudaError_t e = idg::launch_sep3d(cube, out, nx, ny, nz, r[0], r[1], r[2], wt[0], wt[1], wt[2], st);
+        const char *name;
+        const cudaError_t e = run_sep3d(cube, out, nx, ny, nz, r, wt[0], wt[1], wt[2], st, &name);
         if (e != cudaSuccess) return (int)e;
         t_launches = 1;
-        snprintf(t_plan, sizeof(t_plan), "idg_sep3d_kernel gauss r=%d,%d,%d", r[0], r[1], r[2]);
+        snprintf(t_plan, sizeof(t_plan), "%s gauss r=%d,%d,%d", name, r[0], r[1], r[2]);
         return IDG_OK;
     }
     // Eq. 3: K(p) = G(R^-1 p), R = Rz Ry Rx (right-handed, degrees), sampled on the cube |p_j| <= r

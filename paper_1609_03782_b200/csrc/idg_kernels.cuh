@@ -122,6 +122,10 @@ constexpr int kSepMaxRadius = 16;      // per-axis radius limit of the separable
 constexpr int kConvMaxRadius = 10;     // radius limit of the dense kernel (cube support (2r+1)^3)
 cudaError_t launch_sep3d(const float *in, float *out, int nx, int ny, int nz, int rx, int ry, int rz,
                          const float *wx, const float *wy, const float *wz, cudaStream_t st);
+// TMA-fed barrier-free variant for radii <= 4, nx % 4 == 0, 16-byte aligned cubes (idg_sep3d_tma.cu)
+bool sep3d_tma_supported(int nx, int ny, int nz, int rx, int ry, int rz, const void *in, const void *out);
+cudaError_t launch_sep3d_tma(const float *in, float *out, int nx, int ny, int nz, int rx, int ry, int rz,
+                             const float *wx, const float *wy, const float *wz, int zchunk, int variant, cudaStream_t st);
 // kern [device]: (2r+1)^3 weights, x fastest
 cudaError_t launch_conv3d(const float *in, float *out, int nx, int ny, int nz, int r, const float *kern,
                           cudaStream_t st);

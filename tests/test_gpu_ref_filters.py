@@ -73,6 +73,58 @@ def test_gaussian_rotated(B, oracle, shape, case):
     assert B.idg_gaussian_radii(fwhm, theta) == oracle.gaussian_radii_oracle(fwhm, theta)
 
 
+@pytest.fixture
+def sep_plan(B):
+    def set_plan(kernel=0, tile=0, zchunk=0):
+        B.idg_set_option(B.IDG_OPT_KERNEL, kernel)
+        B.idg_set_option(B.IDG_OPT_TILE, tile)
+        B.idg_set_option(B.IDG_OPT_ZCHUNK, zchunk)
+    yield set_plan
+    set_plan()
+
+
+@pytest.mark.parametrize("variant", [0, 2])
+@pytest.mark.parametrize("shape", [(11, 75, 268), (23, 9, 128), (2, 40, 8), (1, 3, 4), (30, 130, 120)], ids=IDS)
+def test_sep3d_tma_kernel_variants(B, oracle, sep_plan, shape, variant):
+    """The TMA-fed separable kernel (radii <= 4, nx % 4 == 0): every radius class in xy and z, both strip heights,
+    several tile columns / rows with ragged tails, cubes smaller than one tile or one kernel, forced z chunks; the
+    plan string must name the kernel, and option kernel = 1 must fall back to the general kernel."""
+    a = noisy(shape, 21)
+    t = torch.from_numpy(a).cuda()
+    for zchunk in (0, 3):
+        sep_plan(0, variant, zchunk)
+        for w in ((3, 3, 3), (5, 3, 1), (1, 9, 5), (9, 7, 9), (7, 1, 3)):
+            out = B.idg_box_filter(t, *w)
+            torch.cuda.synchronize()
+            assert B.idg_last_plan().startswith("idg_sep3d_tma_kernel box"), B.idg_last_plan()
+            assert err(out, oracle.box_filter_oracle(a, *w)) <= TOL, (w, zchunk)
+    sep_plan(0, variant, 0)
+    for fwhm in ((3, 3, 3), (2, 3, 1), (1, 0, 3), (3.3, 1.5, 2)):
+        out = B.idg_gaussian_filter(t, fwhm)
+        torch.cuda.synchronize()
+        assert B.idg_last_plan().startswith("idg_sep3d_tma_kernel gauss"), B.idg_last_plan()
+        assert err(out, oracle.gaussian_filter_oracle(a, fwhm)) <= TOL, fwhm
+    sep_plan(1, 0, 0)
+    out = B.idg_box_filter(t, 3, 5, 5)
+    assert B.idg_last_plan().startswith("idg_sep3d_kernel box")
+    assert err(out, oracle.box_filter_oracle(a, 3, 5, 5)) <= TOL
+
+
+def test_sep3d_tma_kernel_is_repeatable_and_close_to_the_general_kernel(B, sep_plan):
+    """Barrier-free stage hand-back (full / empty mbarriers): a race would show as a run-to-run difference.  Against
+    the general kernel the result differs only by the summation order (y, x, z instead of x, y, z)."""
+    g = torch.Generator(device="cuda").manual_seed(5)
+    x = torch.randn((48, 300, 520), device="cuda", generator=g)
+    sep_plan(1)
+    ref = B.idg_gaussian_filter(x, (3, 3, 3))
+    for variant in (0, 2):
+        sep_plan(0, variant)
+        first = B.idg_gaussian_filter(x, (3, 3, 3))
+        assert float((first - ref).abs().max()) <= 2e-6 * float(x.abs().max())
+        for _ in range(4):
+            assert torch.equal(B.idg_gaussian_filter(x, (3, 3, 3)), first)
+
+
 def test_config0_cube_with_the_papers_timing_parameters(B, oracle):
     """The four reference-filter settings the paper times on the config-0 cube."""
     from paper_1609_03782_b200 import synth
