@@ -679,11 +679,12 @@ int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, i
     cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e = cudaSuccess;
     if (wavelet == IDG_WAVELET_HAAR && levels <= 3 && ny <= 65535 * 8 && nz <= 65535 * 8 &&
-        g_opt[IDG_OPT_KERNEL] != 1) {          // Haar blocks are independent: one fused pass (option kernel = 1: per-axis passes)
-        e = idg::launch_haar_filter(cube, out, nx, ny, nz, levels, thr, st);
+        g_opt[IDG_OPT_KERNEL] != 1) {          // Haar blocks are independent: one fused pass (option kernel = 1: per-axis
+        bool warp = false;                     // passes, 2: the shared-memory regions also where a warp could hold a block)
+        e = idg::launch_haar_filter(cube, out, nx, ny, nz, levels, thr, g_opt[IDG_OPT_KERNEL] != 2, &warp, st);
         if (e != cudaSuccess) return (int)e;
         t_launches = 1;
-        snprintf(t_plan, sizeof(t_plan), "idg_haar_filter_kernel levels=%d", levels);
+        snprintf(t_plan, sizeof(t_plan), "%s levels=%d", warp ? "idg_haar_warp_kernel" : "idg_haar_filter_kernel", levels);
         return IDG_OK;
     }
     int launches = 0;

@@ -143,7 +143,7 @@ cudaError_t launch_histogram(const float *cube, int nx, int ny, const int roi[6]
 cudaError_t launch_wavelet_transform(float *a, int nx, int ny, int nz, int wavelet, int levels, bool inverse,
                                      bool two_phase, cudaStream_t st, int *launches);
 cudaError_t launch_haar_filter(const float *in, float *out, int nx, int ny, int nz, int levels, const float *thr,
-                               cudaStream_t st);
+                               bool warp_blocks, bool *used_warp, cudaStream_t st);
 // idg_legall.cu: Le Gall 5/3 thresholding filter with the axes of a level fused (needs ~1.3 cubes of temporary;
 // cudaErrorMemoryAllocation with nothing launched when there is no room).
 cudaError_t launch_legall_filter(const float *in, float *out, int nx, int ny, int nz, int levels, const float *thr,

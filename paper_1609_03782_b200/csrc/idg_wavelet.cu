@@ -11,6 +11,8 @@
 // write.  Threads are laid out with the lattice x index fastest.  The threshold pass is one more
 // elementwise kernel (band level from the trailing zero bits of the indices).  All of it is bound by
 // HBM traffic; level 1 dominates (the level-l lattice holds 8^-(l-1) of the voxels).
+#include <type_traits>
+
 #include "idg_kernels.cuh"
 
 namespace idg {
@@ -337,6 +339,139 @@ __global__ void __launch_bounds__(NT) idg_haar_filter_kernel(const __grid_consta
     }
 }
 
+// ---- the same filter with an 8 x 8 x 8 block per WARP, in registers --------------------------------------------
+// Lane (xh, yp, zp) = (bit 0, bits 1-2, bits 3-4) holds the 4 x 2 x 2 voxels x = 4 xh + a, y = 2 yp + b, z = 2 zp + c
+// of the block: every level-1 pair (x, y and z) lies inside a lane, the level-2 lattice (even indices) leaves each
+// lane the two values a = 0, 2 of (b, c) = (0, 0), whose y / z partners sit in lanes l ^ 2 / l ^ 8, and the level-3
+// lattice (multiples of 4) one value in the lanes with even yp and zp, partners in lanes l ^ 1, l ^ 4, l ^ 16.  A
+// pair across lanes is one shuffle: both lanes evaluate the pair from the same two operands with the expressions of
+// haar_pair, so the result is bit-identical to the shared-memory kernel and to the per-axis passes.  No shared
+// memory, no barrier; 4 LDG.128 + 4 STG.128 per lane (a warp touches whole 32-byte sectors).  Needs nx % 4 == 0
+// and 16-byte aligned cubes.  Safe in place.
+template <bool INV>
+__device__ __forceinline__ float haar_pair_lanes(float mine, bool odd, unsigned xor_mask)
+{
+    const float other = __shfl_xor_sync(0xffffffffu, mine, xor_mask);
+    if (!INV) {                                   // d = odd - even;  c = even + d/2
+        const float e = odd ? other : mine, o = odd ? mine : other;
+        const float d = o - e;
+        return odd ? d : e + 0.5f * d;
+    } else {                                      // even = c - d/2;  odd = d + even
+        const float c = odd ? other : mine, d = odd ? mine : other;
+        const float e = c - 0.5f * d;
+        return odd ? d + e : e;
+    }
+}
+
+__global__ void __launch_bounds__(NT) idg_haar_warp_kernel(const __grid_constant__ HArgs H)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int gx0 = (blockIdx.x * (NT / 32) + warp) * 8, gy0 = blockIdx.y * 8, gz0 = blockIdx.z * 8;
+    if (gx0 >= H.nx) return;                      // warp uniform
+    const int xh = lane & 1, yp = (lane >> 1) & 3, zp = (lane >> 3) & 3;
+    const int gx = gx0 + 4 * xh, gy = gy0 + 2 * yp, gz = gz0 + 2 * zp;
+    const size_t plane = (size_t)H.nx * H.ny;
+    const bool in_x = gx < H.nx;
+    // reading W2: a pair exists if its odd partner lies on the lattice; otherwise the even sample is left alone
+    const bool py1 = gy + 1 < H.ny, pz1 = gz + 1 < H.nz;
+    const bool py2 = gy0 + 4 * (yp >> 1) + 2 < H.ny, pz2 = gz0 + 4 * (zp >> 1) + 2 < H.nz;
+    const bool px3 = gx0 + 4 < H.nx, py3 = gy0 + 4 < H.ny, pz3 = gz0 + 4 < H.nz;
+    const bool on3 = !(yp & 1) && !(zp & 1);      // this lane holds a level-3 lattice point (a = b = c = 0)
+
+    float v[2][2][4];
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+            float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (in_x && gy + b < H.ny && gz + c < H.nz)
+                t = __ldg(reinterpret_cast<const float4 *>(H.in + (size_t)(gz + c) * plane + (size_t)(gy + b) * H.nx + gx));
+            v[c][b][0] = t.x; v[c][b][1] = t.y; v[c][b][2] = t.z; v[c][b][3] = t.w;
+        }
+
+    auto level1 = [&](auto inv) {
+        constexpr bool INV = decltype(inv)::value;
+        auto xs = [&]() {                         // lines outside the cube hold zeros and stay zero
+#pragma unroll
+            for (int c = 0; c < 2; ++c)
+#pragma unroll
+                for (int b = 0; b < 2; ++b) {
+                    haar_pair<INV>(v[c][b][0], v[c][b][1]);
+                    haar_pair<INV>(v[c][b][2], v[c][b][3]);
+                }
+        };
+        auto ys = [&]() {
+            if (py1) {
+#pragma unroll
+                for (int c = 0; c < 2; ++c)
+#pragma unroll
+                    for (int a = 0; a < 4; ++a) haar_pair<INV>(v[c][0][a], v[c][1][a]);
+            }
+        };
+        auto zs = [&]() {
+            if (pz1) {
+#pragma unroll
+                for (int b = 0; b < 2; ++b)
+#pragma unroll
+                    for (int a = 0; a < 4; ++a) haar_pair<INV>(v[0][b][a], v[1][b][a]);
+            }
+        };
+        if (!INV) { xs(); ys(); zs(); } else { zs(); ys(); xs(); }
+    };
+    auto level2 = [&](auto inv) {
+        constexpr bool INV = decltype(inv)::value;
+        float &u0 = v[0][0][0], &u1 = v[0][0][2];
+        auto xs = [&]() { haar_pair<INV>(u0, u1); };
+        auto ys = [&]() {
+            const float a0 = haar_pair_lanes<INV>(u0, yp & 1, 2), a1 = haar_pair_lanes<INV>(u1, yp & 1, 2);
+            if (py2) { u0 = a0; u1 = a1; }
+        };
+        auto zs = [&]() {
+            const float a0 = haar_pair_lanes<INV>(u0, zp & 1, 8), a1 = haar_pair_lanes<INV>(u1, zp & 1, 8);
+            if (pz2) { u0 = a0; u1 = a1; }
+        };
+        if (!INV) { xs(); ys(); zs(); } else { zs(); ys(); xs(); }
+    };
+    auto level3 = [&](auto inv) {
+        constexpr bool INV = decltype(inv)::value;
+        float &u = v[0][0][0];
+        auto xs = [&]() { const float a = haar_pair_lanes<INV>(u, xh, 1); if (on3 && px3) u = a; };
+        auto ys = [&]() { const float a = haar_pair_lanes<INV>(u, (yp >> 1) & 1, 4); if (on3 && py3) u = a; };
+        auto zs = [&]() { const float a = haar_pair_lanes<INV>(u, (zp >> 1) & 1, 16); if (on3 && pz3) u = a; };
+        if (!INV) { xs(); ys(); zs(); } else { zs(); ys(); xs(); }
+    };
+
+    level1(std::false_type{});
+    if (H.levels >= 2) level2(std::false_type{});
+    if (H.levels >= 3) level3(std::false_type{});
+    // hard thresholds by band (reading W3): level of a coefficient = trailing zero bits of its indices + 1, capped
+    const float t1 = H.thr[0];
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int b = 0; b < 2; ++b)
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                float t = t1;
+                if (c == 0 && b == 0 && (a & 1) == 0) {
+                    const int tz = __ffs((4 * xh + a) | (2 * yp) | (2 * zp) | 8) - 1;
+                    t = H.thr[(tz + 1 < H.levels ? tz + 1 : H.levels) - 1];
+                }
+                if (fabsf(v[c][b][a]) < t) v[c][b][a] = 0.f;
+            }
+    if (H.levels >= 3) level3(std::true_type{});
+    if (H.levels >= 2) level2(std::true_type{});
+    level1(std::true_type{});
+
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int b = 0; b < 2; ++b)
+            if (in_x && gy + b < H.ny && gz + c < H.nz)
+                *reinterpret_cast<float4 *>(H.out + (size_t)(gz + c) * plane + (size_t)(gy + b) * H.nx + gx) =
+                    make_float4(v[c][b][0], v[c][b][1], v[c][b][2], v[c][b][3]);
+}
+
 template <int WAVELET, int PHASE, bool INV>
 cudaError_t launch_phase(const WArgs &W, cudaStream_t st)
 {
@@ -417,16 +552,20 @@ cudaError_t launch_wavelet_transform(float *a, int nx, int ny, int nz, int wavel
                         : transform<1>(a, nx, ny, nz, levels, inverse, two_phase, st, launches);
 }
 
-// Haar, 1..3 levels: the fused single-pass filter.  thr[l-1] = t_l * rms.
+// Haar, 1..3 levels: the fused single-pass filter.  thr[l-1] = t_l * rms.  warp_blocks: an 8^3 block per warp in
+// registers where the cube allows float4 access (*used_warp reports it), else 64 x 8 x 8 regions in shared memory.
 cudaError_t launch_haar_filter(const float *in, float *out, int nx, int ny, int nz, int levels, const float *thr,
-                               cudaStream_t st)
+                               bool warp_blocks, bool *used_warp, cudaStream_t st)
 {
     if (levels < 1 || levels > 3) return cudaErrorInvalidValue;
     HArgs H{in, out, nx, ny, nz, levels, {0.f, 0.f, 0.f}};
     for (int i = 0; i < levels; ++i) H.thr[i] = thr[i];
     const unsigned gx = (unsigned)((nx + HX - 1) / HX), gy = (unsigned)((ny + HY - 1) / HY), gz = (unsigned)((nz + HZ - 1) / HZ);
     if (gy > 65535u || gz > 65535u) return cudaErrorInvalidValue;
-    idg_haar_filter_kernel<<<dim3(gx, gy, gz), NT, 0, st>>>(H);
+    const bool vec = (nx % 4 == 0) && ((((uintptr_t)in | (uintptr_t)out) & 15u) == 0);
+    *used_warp = warp_blocks && vec;
+    if (*used_warp) idg_haar_warp_kernel<<<dim3(gx, gy, gz), NT, 0, st>>>(H);      // 8 warps = 64 columns, as the regions
+    else idg_haar_filter_kernel<<<dim3(gx, gy, gz), NT, 0, st>>>(H);
     return cudaGetLastError();
 }
 

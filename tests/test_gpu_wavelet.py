@@ -79,21 +79,28 @@ def test_filter(B, oracle, shape, wavelet, thr):
         assert np.abs(out - oracle.wavelet_filter_oracle(a, wavelet, [float(np.float32(t)) for t in thr], rms)).max() <= TOL * rms
 
 
-@pytest.mark.parametrize("shape", SHAPES + [(8, 8, 32), (17, 23, 77), (64, 72, 160)], ids=IDS)
+@pytest.mark.parametrize("shape", SHAPES + [(8, 8, 32), (17, 23, 77), (64, 72, 160), (21, 67, 100), (13, 30, 268),
+                                            (9, 5, 12), (17, 23, 76), (3, 2, 4)], ids=IDS)
 def test_haar_fused_pass_equals_per_axis_passes(B, shape):
-    """The single-pass Haar filter (8^3 blocks in shared memory) applies the same operations in the same order as
-    the per-level, per-axis kernels: bit-identical for every shape (odd extents, regions hanging over the faces),
-    1..3 levels, in place or not."""
+    """The single-pass Haar filters (an 8^3 block per warp in registers where nx % 4 == 0, else 64 x 8 x 8 regions in
+    shared memory; option kernel = 2 forces the latter) apply the same operations in the same order as the
+    per-level, per-axis kernels: bit-identical for every shape (odd extents, blocks hanging over the faces), 1..3
+    levels, in place or not."""
     a = torch.from_numpy(noisy(shape, 23)).cuda()
     for thr in ((0.7,), (0.5, 0.8), (0.5, 0.8, 1.1), (0.0, 0.0, 0.0)):
         B.idg_set_option(B.IDG_OPT_KERNEL, 1)
         try:
             ref = B.idg_wavelet_filter(a, B.WAVELET_HAAR, thr, 1.3)
             plan_ref = B.idg_last_plan()
+            assert "idg_lift_kernel" in plan_ref
+            B.idg_set_option(B.IDG_OPT_KERNEL, 2)
+            out = B.idg_wavelet_filter(a, B.WAVELET_HAAR, thr, 1.3)
+            assert "idg_haar_filter_kernel" in B.idg_last_plan()
+            assert torch.equal(out, ref), (shape, thr)
         finally:
             B.idg_set_option(B.IDG_OPT_KERNEL, 0)
         out = B.idg_wavelet_filter(a, B.WAVELET_HAAR, thr, 1.3)
-        assert "idg_haar_filter_kernel" in B.idg_last_plan() and "idg_lift_kernel" in plan_ref
+        assert ("idg_haar_warp_kernel" if shape[2] % 4 == 0 else "idg_haar_filter_kernel") in B.idg_last_plan()
         assert torch.equal(out, ref), (shape, thr)
         inplace = a.clone()
         B.idg_wavelet_filter(inplace, B.WAVELET_HAAR, thr, 1.3, out=inplace)
