@@ -249,7 +249,9 @@ int idg_wavelet_transform(const float *cube, int nx, int ny, int nz, int wavelet
  * Le Gall 5/3: the default path fuses the three axes of a level and works out of place on compact lattices in a
  * stream-ordered temporary of ~1.3 cubes (see idg_release_temporaries); when that cannot be allocated, or with
  * IDG_OPT_KERNEL = 2 (1: two-phase passes), it runs the in-place passes, which need no memory ("does not require
- * additional memory").  All paths give bit-identical results.
+ * additional memory").  Haar, levels <= 3: one fused pass (an 8 x 8 x 8 block per warp in registers when
+ * nx % 4 == 0 and the cubes are 16-byte aligned, else -- or with IDG_OPT_KERNEL = 2 -- 64 x 8 x 8 regions in shared
+ * memory; IDG_OPT_KERNEL = 1: the in-place passes).  All paths give bit-identical results.
  */
 int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, int levels, const float *thresholds,
                        float rms, float *out, void *stream);
@@ -258,7 +260,8 @@ int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, i
  * Process-wide tuning knobs (tests and benchmarks; defaults give the fastest plan).
  *   IDG_OPT_KERNEL   0 auto (kernel 3 wherever nx % 4 == 0 and the buffers are 16-byte aligned) | 1 naive (one
  *                    thread per voxel) | 2 tiled z-streaming kernel (global loads) | 3 tiled z-streaming kernel
- *                    fed by TMA (the fast path) | 4 persistent warp-decoupled TMA kernel
+ *                    fed by TMA (the fast path) | 4 persistent warp-decoupled TMA kernel.  Reference filters: 1 = the
+ *                    general separable kernel also where the TMA-fed one applies.  Wavelets: see idg_wavelet_filter
  *   IDG_OPT_FUSE     0 auto (4, or 2 for full-GPU workloads of cubes thinner than 100 planes) | 1..4 = diffusion
  *                    iterations fused per launch (kernels 2-4)
  *   IDG_OPT_ZCHUNK   0 auto | >0  = planes per CTA along z (kernels 2, 3)
