@@ -271,10 +271,12 @@ int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, i
  *                    rows per thread instead of 2 in idg_sep3d_tma_kernel
  *   IDG_OPT_CTAS     0 auto | >0  = persistent grid size of kernel 4
  *   IDG_OPT_HOST_SLABS  0 auto | 1..16 = z slabs of the idg_filter_host transfer/compute pipeline (1 = one piece)
+ *   IDG_OPT_COOP     0 auto (small cubes whose whole grid is co-resident: all launches of kernel 3 folded into ONE
+ *                    cooperative launch with grid barriers between the fused rounds) | 1 never | 2 whenever the grid fits
  * idg_get_option returns the current value, or IDG_ERR_OPTION.
  */
 enum { IDG_OPT_KERNEL = 0, IDG_OPT_FUSE = 1, IDG_OPT_ZCHUNK = 2, IDG_OPT_TILE = 3, IDG_OPT_CTAS = 4,
-       IDG_OPT_HOST_SLABS = 5, IDG_OPT_COUNT_ = 6 };
+       IDG_OPT_HOST_SLABS = 5, IDG_OPT_COOP = 6, IDG_OPT_COUNT_ = 7 };
 int idg_set_option(int key, int value);
 int idg_get_option(int key);
 

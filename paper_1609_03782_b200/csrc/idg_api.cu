@@ -12,11 +12,12 @@
 
 namespace {
 
-int g_opt[IDG_OPT_COUNT_] = {0, 0, 0, 0, 0, 0};
+int g_opt[IDG_OPT_COUNT_] = {0, 0, 0, 0, 0, 0, 0};
 thread_local int t_launches = 0;
 thread_local char t_plan[96] = "none";
 
 constexpr size_t kAlign = 256;
+constexpr double kCoopMaxVoxels = 1.5e6;      // auto plan: cooperative single launch up to this many voxels per call
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 bool voxel_count(int nx, int ny, int nz, int batch, size_t *n_one)
@@ -86,6 +87,7 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
 
     float *scratch = (float *)workspace;
     idg::CubeParams *tab = (idg::CubeParams *)((char *)workspace + align_up(bytes));
+    unsigned *coop_bar = (unsigned *)((char *)tab + align_up(sizeof(idg::CubeParams) * (size_t)batch));
 
     // Plan: kernel variant and iterations fused per launch.
     const bool can_tile = idg::tiled_supported(nx, ny, nz, cubes, out, scratch);
@@ -104,6 +106,10 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
         const double work = (double)N * (double)batch;
         if (can_tma) {
             kernel = 3;
+            // Small cubes: a round costs ~10 us (T = 3) to ~14 us (T = 4) whatever the cube, so three iterations per
+            // round, all rounds in one cooperative launch, beat four per launch from five iterations on
+            // (profiles/r1k_notes.md).
+            if (!fuse && work <= kCoopMaxVoxels && g_opt[IDG_OPT_COOP] != 1 && max_n >= 5) fuse = 3;
             if (!fuse) fuse = (nz < 100 && work >= 4.0e6) ? 2 : 4;
         } else {
             kernel = can_tile ? 2 : 1;
@@ -177,6 +183,24 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
         e = cudaMemcpyAsync(scratch, cubes, bytes, cudaMemcpyDeviceToDevice, st);
         if (e != cudaSuccess) return (int)e;
     }
+    // Small cubes (launch latency and prologue dominate a launch): all rounds in ONE cooperative launch if the whole
+    // grid is co-resident.  Measured on B200 (profiles/r1k_notes.md).
+    const int rounds = (max_n + fuse - 1) / fuse;
+    const int coop = g_opt[IDG_OPT_COOP];
+    if (kernel == 3 && mode == 0 && rounds >= 2 && coop != 1 &&
+        (coop == 2 || (double)N * (double)batch <= kCoopMaxVoxels)) {
+        e = cudaMemsetAsync(coop_bar, 0, 8, st);
+        if (e != cudaSuccess) return (int)e;
+        L.iter_done = 0;
+        e = idg::launch_tma_coop(L, g_opt[IDG_OPT_ZCHUNK], tile, rounds, coop_bar, st);
+        if (e == cudaSuccess) {
+            t_launches = 1;
+            snprintf(t_plan, sizeof(t_plan), "idg_tma_coop_kernel fuse=%d rounds=%d", fuse, rounds);
+            return IDG_OK;
+        }
+        if (e != cudaErrorNotSupported && e != cudaErrorCooperativeLaunchTooLarge) return (int)e;
+        (void)cudaGetLastError();           // does not fit: one launch per round
+    }
     for (int done = 0; done < max_n; done += fuse) {
         L.iter_done = done;
         int tile_now = tile;
@@ -234,7 +258,8 @@ size_t idg_workspace_bytes(int nx, int ny, int nz, int batch)
 {
     size_t N;
     if (!voxel_count(nx, ny, nz, batch, &N)) return 0;
-    return align_up(N * (size_t)batch * sizeof(float)) + align_up(sizeof(idg::CubeParams) * (size_t)batch);
+    return align_up(N * (size_t)batch * sizeof(float)) + align_up(sizeof(idg::CubeParams) * (size_t)batch) +
+           kAlign;      // scratch cubes | per-cube constants | arrival counter of the cooperative launch
 }
 
 int idg_filter_ws(const float *cube, int nx, int ny, int nz, int n_iter, const idg_params *params,
@@ -720,6 +745,7 @@ int idg_set_option(int key, int value)
     if (key == IDG_OPT_TILE && (value < 0 || value > 4)) return IDG_ERR_OPTION;
     if (key == IDG_OPT_CTAS && value < 0) return IDG_ERR_OPTION;
     if (key == IDG_OPT_HOST_SLABS && (value < 0 || value > kMaxSlabs)) return IDG_ERR_OPTION;
+    if (key == IDG_OPT_COOP && (value < 0 || value > 2)) return IDG_ERR_OPTION;
     g_opt[key] = value;
     return IDG_OK;
 }

@@ -36,21 +36,26 @@ struct Launch {
 
 // Which buffers cube b reads / writes in this launch so that its LAST launch writes `out`.
 // Returns the number of iterations to apply now (0 = cube already finished).
-__device__ __forceinline__ int route(const Launch &L, int b, const CubeParams &p,
+// iter_done: iterations applied before this launch (L.iter_done), or before this round of a cooperative launch.
+__device__ __forceinline__ int route(const Launch &L, int iter_done, int b, const CubeParams &p,
                                      const float *&src, float *&dst)
 {
-    const int remaining = p.n_iter - L.iter_done;
+    const int remaining = p.n_iter - iter_done;
     if (remaining <= 0) return 0;
     const int now = remaining < L.fuse ? remaining : L.fuse;
     const int after = (remaining - now + L.fuse - 1) / L.fuse;      // launches still to come
     const size_t off = (size_t)b * (size_t)L.nx * (size_t)L.ny * (size_t)L.nz;
     float *o = L.out + off, *s = L.scratch + off;
     dst = (after & 1) ? s : o;
-    if (L.iter_done == 0)   // first launch: read I_0 (from the staged copy if it would alias dst)
+    if (iter_done == 0)     // first launch: read I_0 (from the staged copy if it would alias dst)
         src = (L.in_place && !(after & 1)) ? s : (L.in + off);
     else
         src = (after & 1) ? o : s;
     return now;
+}
+__device__ __forceinline__ int route(const Launch &L, int b, const CubeParams &p, const float *&src, float *&dst)
+{
+    return route(L, L.iter_done, b, p, src, dst);
 }
 
 __device__ __forceinline__ CubeParams cube_params(const Launch &L, int b)
@@ -100,6 +105,10 @@ cudaError_t launch_naive(const Launch &L, cudaStream_t st);
 cudaError_t launch_tiled(const Launch &L, int zchunk, cudaStream_t st);
 bool tiled_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
 cudaError_t launch_tma(const Launch &L, int zchunk, int tile, cudaStream_t st);
+// All `rounds` launches of a plan (fuse iterations each) as ONE cooperative launch with grid barriers in between, for
+// workloads whose whole grid is co-resident (small, L2-resident cubes).  bar: 8 zeroed bytes of device memory.
+// cudaErrorNotSupported / cudaErrorCooperativeLaunchTooLarge: use launch_tma per round instead.
+cudaError_t launch_tma_coop(const Launch &L, int zchunk, int tile, int rounds, unsigned *bar, cudaStream_t st);
 bool tma_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
 cudaError_t launch_stream(const Launch &L, int nctas, int tile, cudaStream_t st);
 bool stream_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);

@@ -41,6 +41,10 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
 }
+__device__ __forceinline__ void mbar_inval(uint32_t bar)
+{
+    asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
 __device__ __forceinline__ void mbar_fence_init()
 {
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -91,6 +95,26 @@ __device__ __forceinline__ uint32_t atom_add_relaxed(uint32_t addr, uint32_t v)
     uint32_t old;
     asm volatile("atom.relaxed.cta.shared::cta.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(addr), "r"(v) : "memory");
     return old;
+}
+// Grid-wide barrier for cooperative launches (all CTAs co-resident): `bar` counts arrivals monotonically, `target`
+// = CTAs x barriers passed so far.  Global data written before it by any CTA (generic proxy) may afterwards be read
+// by any CTA, also through TMA (async proxy).
+__device__ __forceinline__ void grid_barrier(unsigned *bar, unsigned target)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        asm volatile("fence.proxy.async.global;" ::: "memory");
+        atomicAdd(bar, 1u);
+        unsigned v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+        } while (v < target);
+        __threadfence();
+        asm volatile("fence.proxy.async.global;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
 }
 __device__ __forceinline__ void sts32(uint32_t addr, uint32_t v)
 {

@@ -103,6 +103,8 @@ struct TmaArgs {
     int tiles_x, tiles_y;
     int zchunk;
     int halo;
+    int rounds;            // cooperative launch: launches folded into this one (else 1)
+    unsigned *bar;         // cooperative launch: arrival counter of the grid barrier (zeroed by the host)
 };
 
 struct Maps {
@@ -124,7 +126,7 @@ struct Smem {
 template <int TL, int R, int WARPS, int NS, int TMAX, bool ONE>
 __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restrict__ dst, const Launch &L,
                                          const TmaArgs &A, const CubeParams &prm, int b,
-                                         unsigned char *smem)
+                                         unsigned char *smem, bool reinit = false)
 {
     using S = Smem<TMAX, R, WARPS, NS>;
     constexpr int TILE_Y = WARPS * R;
@@ -179,7 +181,10 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
 
     if (threadIdx.x == 0) {
 #pragma unroll
-        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+        for (int s = 0; s < NS; ++s) {
+            if (reinit) ptx::mbar_inval(ptx::smem_u32(&full[s]));      // a later round of a cooperative launch
+            mbar_init(&full[s], 1);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -313,18 +318,52 @@ idg_tma_kernel(const __grid_constant__ Launch L, const __grid_constant__ TmaArgs
     else if (T > 3 && now == 3) tma_body<(T > 3 ? 3 : 1), R, WARPS, NS, T, ONE>(map, dst, L, A, prm, b, smem);
 }
 
+// Cooperative variant: all `A.rounds` launches of a plan in one, a grid barrier between rounds (the whole grid is
+// co-resident); for small, L2-resident cubes, whose launches are bound by launch latency and the prologue.
+template <int T, int R, int WARPS, int NS, int MINB, bool ONE>
+__global__ void __launch_bounds__(WARPS * 32, MINB)
+idg_tma_coop_kernel(const __grid_constant__ Launch L, const __grid_constant__ TmaArgs A,
+               const __grid_constant__ Maps M)
+{
+    extern __shared__ __align__(1024) unsigned char smem[];
+    const int b = blockIdx.z;
+    const CubeParams prm = cube_params(L, b);
+    const size_t off = (size_t)b * (size_t)L.nx * (size_t)L.ny * (size_t)L.nz;
+    constexpr bool COOP = true;
+    const int rounds = A.rounds;
+    const unsigned ctas = gridDim.x * gridDim.y * gridDim.z;
+    for (int round = 0; round < rounds; ++round) {
+        const float *src;
+        float *dst;
+        const int now = route(L, L.iter_done + round * L.fuse, b, prm, src, dst);
+        if (now > 0) {
+            const CUtensorMap *map = (src == L.scratch + off) ? &M.scratch : (src == L.out + off) ? &M.out : &M.in;
+            const bool re = COOP && round > 0;
+            if (now == T) tma_body<T, R, WARPS, NS, T, ONE>(map, dst, L, A, prm, b, smem, re);
+            else if (T > 1 && now == 1) tma_body<1, R, WARPS, NS, T, ONE>(map, dst, L, A, prm, b, smem, re);
+            else if (T > 2 && now == 2) tma_body<(T > 2 ? 2 : 1), R, WARPS, NS, T, ONE>(map, dst, L, A, prm, b, smem, re);
+            else if (T > 3 && now == 3) tma_body<(T > 3 ? 3 : 1), R, WARPS, NS, T, ONE>(map, dst, L, A, prm, b, smem, re);
+        } else if (!COOP) {
+            return;
+        }
+        if (COOP && round + 1 < rounds) ptx::grid_barrier(A.bar, ctas * (unsigned)(round + 1));
+    }
+}
+
 bool encode_map(CUtensorMap *m, const float *base, const Launch &L, int tile_y)
 {
     return tmap_encode(m, base, L.nx, L.ny, L.nz, L.batch, kTileX, tile_y);
 }
 
-int pick_zchunk(int nz, long tiles, int T, int slots)
+// max_ctas > 0: only chunkings whose whole grid is at most max_ctas CTAs (cooperative launch); 0 if none is.
+int pick_zchunk(int nz, long tiles, int T, int slots, long max_ctas = 0)
 {
     long best_cost = -1;
-    int best = nz;
+    int best = max_ctas > 0 ? 0 : nz;
     for (int nchunks = 1; nchunks <= nz; ++nchunks) {
         const int zc = (nz + nchunks - 1) / nchunks;
         const long ctas = tiles * ((nz + zc - 1) / zc);
+        if (max_ctas > 0 && ctas > max_ctas) break;
         const long waves = (ctas + slots - 1) / slots;
         const long cost = waves * (zc + 2 * T + 3);      // +3: prologue and pipeline fill, in plane-steps
         if (best_cost < 0 || cost < best_cost) {
@@ -336,34 +375,69 @@ int pick_zchunk(int nz, long tiles, int T, int slots)
     return best;
 }
 
-template <int T, int R, int WARPS, int NS, int MINB>
-cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st)
+int sm_count()
+{
+    static int n = 0;
+    if (!n) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+            n = 0;
+    }
+    return n;
+}
+
+// rounds > 1: cooperative launch of all rounds (COOP instantiation); the grid must be co-resident.
+template <int T, int R, int WARPS, int NS, int MINB, bool COOP = false>
+cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st, int rounds = 1, unsigned *bar = nullptr)
 {
     using S = Smem<T, R, WARPS, NS>;
     constexpr int TILE_Y = WARPS * R;
     static_assert(TILE_Y > 2 * T, "tile must be taller than its halo");
     static_assert(S::kBytes * MINB <= 227 * 1024, "shared memory budget");
+    constexpr bool coop = COOP;
     TmaArgs A;
     A.halo = T;
+    A.rounds = rounds;
+    A.bar = bar;
     const bool one = L.nx <= kTileX;                     // a single tile column: no halo lanes
     A.tiles_x = one ? 1 : (L.nx / 4 + kValidLanes - 1) / kValidLanes;
     A.tiles_y = (L.ny + (TILE_Y - 2 * T) - 1) / (TILE_Y - 2 * T);
     const long tiles = (long)A.tiles_x * A.tiles_y;
     if (tiles > 0x7fffffffL) return cudaErrorInvalidValue;
-    A.zchunk = zchunk > 0 ? (zchunk < L.nz ? zchunk : L.nz) : pick_zchunk(L.nz, tiles * L.batch, T, 148 * MINB);
-    if ((L.nz + A.zchunk - 1) / A.zchunk > 65535) A.zchunk = (L.nz + 65534) / 65535;
-    Maps M;
-    if (!encode_map(&M.in, L.in, L, TILE_Y) || !encode_map(&M.out, L.out, L, TILE_Y) ||
-        !encode_map(&M.scratch, L.scratch, L, TILE_Y))
-        return cudaErrorNotSupported;
-    auto kern = one ? idg_tma_kernel<T, R, WARPS, NS, MINB, true> : idg_tma_kernel<T, R, WARPS, NS, MINB, false>;
+    void (*kern)(Launch, TmaArgs, Maps);
+    if constexpr (COOP) kern = one ? idg_tma_coop_kernel<T, R, WARPS, NS, MINB, true> : idg_tma_coop_kernel<T, R, WARPS, NS, MINB, false>;
+    else kern = one ? idg_tma_kernel<T, R, WARPS, NS, MINB, true> : idg_tma_kernel<T, R, WARPS, NS, MINB, false>;
     static bool attr_done[2] = {false, false};
     if (!attr_done[one]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::kBytes);
         if (e != cudaSuccess) return e;
         attr_done[one] = true;
     }
+    long slots = 148L * MINB;
+    if (coop) {
+        static int per_sm[2] = {-1, -1};
+        if (per_sm[one] < 0 &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[one], kern, WARPS * 32, S::kBytes) != cudaSuccess)
+            per_sm[one] = 0;
+        slots = (long)per_sm[one] * sm_count();
+        if (slots <= 0 || tiles * L.batch > slots) return cudaErrorCooperativeLaunchTooLarge;
+        A.zchunk = pick_zchunk(L.nz, tiles * L.batch, T, (int)slots, slots);
+        if (zchunk > 0 && tiles * L.batch * ((L.nz + zchunk - 1) / zchunk) <= slots) A.zchunk = zchunk < L.nz ? zchunk : L.nz;
+        if (A.zchunk <= 0) return cudaErrorCooperativeLaunchTooLarge;
+    } else {
+        A.zchunk = zchunk > 0 ? (zchunk < L.nz ? zchunk : L.nz) : pick_zchunk(L.nz, tiles * L.batch, T, 148 * MINB);
+    }
+    if ((L.nz + A.zchunk - 1) / A.zchunk > 65535) A.zchunk = (L.nz + 65534) / 65535;
+    Maps M;
+    if (!encode_map(&M.in, L.in, L, TILE_Y) || !encode_map(&M.out, L.out, L, TILE_Y) ||
+        !encode_map(&M.scratch, L.scratch, L, TILE_Y))
+        return cudaErrorNotSupported;
     dim3 grid((unsigned)tiles, (unsigned)((L.nz + A.zchunk - 1) / A.zchunk), (unsigned)L.batch);
+    if (coop) {
+        if ((long)grid.x * grid.y * grid.z > slots) return cudaErrorCooperativeLaunchTooLarge;
+        void *args[3] = {(void *)&L, (void *)&A, (void *)&M};
+        return cudaLaunchCooperativeKernel((const void *)kern, grid, dim3(WARPS * 32), args, S::kBytes, st);
+    }
     kern<<<grid, WARPS * 32, S::kBytes, st>>>(L, A, M);
     return cudaGetLastError();
 }
@@ -401,6 +475,19 @@ cudaError_t launch_tma(const Launch &L, int zchunk, int tile, cudaStream_t st)
         default: return launch_cfg<4, 4, 8, 4, 1>(L, zchunk, st);
         }
     default: return cudaErrorInvalidValue;
+    }
+}
+
+// The default tilings only: T = 2 on two CTAs per SM, T = 3 / T = 4 on one 8-warp CTA per SM.
+cudaError_t launch_tma_coop(const Launch &L, int zchunk, int tile, int rounds, unsigned *bar, cudaStream_t st)
+{
+    (void)tile;
+    if (rounds < 2 || !bar) return cudaErrorNotSupported;
+    switch (L.fuse) {
+    case 2: return launch_cfg<2, 4, 8, 4, 2, true>(L, zchunk, st, rounds, bar);
+    case 3: return launch_cfg<3, 4, 8, 4, 1, true>(L, zchunk, st, rounds, bar);
+    case 4: return launch_cfg<4, 4, 8, 4, 1, true>(L, zchunk, st, rounds, bar);
+    default: return cudaErrorNotSupported;
     }
 }
 

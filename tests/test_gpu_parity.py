@@ -23,7 +23,7 @@ def B():
     binding.lib()           # fails loudly if the extension is missing
     yield binding
     for k in (binding.IDG_OPT_KERNEL, binding.IDG_OPT_FUSE, binding.IDG_OPT_ZCHUNK, binding.IDG_OPT_TILE,
-              binding.IDG_OPT_CTAS):
+              binding.IDG_OPT_CTAS, binding.IDG_OPT_COOP):
         binding.idg_set_option(k, 0)
 
 
@@ -34,7 +34,10 @@ PLAN_IDS = ["naive", "tiled-T1", "tiled-T2", "tiled-T3", "tiled-T4", "tma-T1", "
             "stream-T1", "stream-T2", "stream-T3", "stream-T4", "auto"]
 
 
-def set_plan(B, plan, zchunk=0, tile=0, ctas=0):
+def set_plan(B, plan, zchunk=0, tile=0, ctas=0, coop=None):
+    """Forced plans run one launch per fused round (coop = 1), as the large cubes do; the auto plan (0, 0) keeps the
+    library default, which folds the rounds of small cubes into one cooperative launch."""
+    B.idg_set_option(B.IDG_OPT_COOP, (0 if tuple(plan) == (0, 0) else 1) if coop is None else coop)
     B.idg_set_option(B.IDG_OPT_KERNEL, plan[0])
     B.idg_set_option(B.IDG_OPT_FUSE, plan[1])
     B.idg_set_option(B.IDG_OPT_ZCHUNK, zchunk)
@@ -378,6 +381,61 @@ def test_launch_count(B):
         set_plan(B, (k, 2))
         B.idg_filter(t, 7)
         assert B.idg_last_launch_count() == 4
+
+
+@pytest.mark.parametrize("fuse", [2, 3, 4])
+@pytest.mark.parametrize("shape", [(67, 100, 100), (20, 70, 264), (9, 33, 128), (40, 130, 520), (3, 5, 8)],
+                         ids=lambda s: "x".join(map(str, s[::-1])))
+def test_cooperative_single_launch_is_bitwise_equal_to_one_launch_per_round(B, oracle, shape, fuse):
+    """IDG_OPT_COOP = 2: all rounds of kernel 3 in ONE cooperative launch with grid barriers in between (the path small
+    cubes take by default).  Same kernels' arithmetic, so the result must equal the launch-per-round path bit for
+    bit, on every run (a missing fence between a round's stores and the next round's TMA loads would show), for n
+    that is and is not a multiple of T, in place, and within the oracle tolerance."""
+    g = torch.Generator(device="cuda").manual_seed(7)
+    x = torch.randn(shape, device="cuda", generator=g) * 2.0
+    p = B.Params(K=1.5, tau=0.03, cx=5.0, cy=4.0, cz=6.0, rms=1.0)
+    for n in (2 * fuse, 2 * fuse + 1, 10):
+        set_plan(B, (3, fuse), coop=1)
+        ref = B.idg_filter(x, n, p)
+        launches = B.idg_last_launch_count()
+        for rep in range(3):
+            set_plan(B, (3, fuse), coop=2)
+            out = B.idg_filter(x, n, p)
+            torch.cuda.synchronize()
+            if "coop" in B.idg_last_plan():
+                assert B.idg_last_launch_count() == 1 and launches > 1
+            assert torch.equal(out, ref), (shape, fuse, n, rep, int((out != ref).sum()))
+        inplace = x.clone()
+        B.idg_filter(inplace, n, p, out=inplace)
+        assert torch.equal(inplace, ref)
+    if x.numel() < 1_000_000:
+        want = oracle.idg_filter_oracle(x.cpu().numpy(), 10, **p.f32())
+        assert err(out.cpu().numpy(), want, 1.0) <= TOL
+
+
+def test_cooperative_launch_batched_mixed_iteration_counts(B, oracle):
+    """Per-cube iteration counts inside one cooperative launch: cubes that have finished keep arriving at the grid
+    barriers; each cube equals its single-cube result."""
+    g = torch.Generator(device="cuda").manual_seed(8)
+    xs = torch.randn((5, 16, 40, 128), device="cuda", generator=g)
+    ns = [0, 3, 10, 7, 4]
+    ps = [B.Params(K=1.0 + 0.5 * b) for b in range(5)]
+    set_plan(B, (3, 4), coop=2)
+    out = B.idg_filter_batched(xs, ns, ps)
+    assert "coop" in B.idg_last_plan()
+    for b in range(5):
+        set_plan(B, (1, 0))
+        assert torch.equal(out[b], B.idg_filter(xs[b], ns[b], ps[b])), b
+
+
+def test_auto_plan_uses_the_cooperative_launch_for_small_cubes_only(B):
+    set_plan(B, (0, 0))
+    B.idg_filter(torch.zeros(67, 100, 100, device="cuda"), 10)
+    assert "idg_tma_coop_kernel" in B.idg_last_plan() and B.idg_last_launch_count() == 1
+    B.idg_filter(torch.zeros(128, 512, 512, device="cuda"), 8)
+    assert "idg_tma_kernel" in B.idg_last_plan() and B.idg_last_launch_count() == 2
+    B.idg_filter(torch.zeros(8, 16, 16, device="cuda"), 3)          # one round: nothing to fold
+    assert "idg_tma_kernel" in B.idg_last_plan()
 
 
 @pytest.mark.parametrize("plan", [(2, 2), (3, 1), (3, 2), (3, 3), (3, 4), (4, 1), (4, 2), (4, 3), (4, 4)],
