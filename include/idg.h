@@ -81,7 +81,8 @@ unsigned idg_params_check(const idg_params *params /*[host]*/);
 /*
  * Bytes of device workspace idg_filter_ws / idg_filter_batched need for `batch`
  * cubes of nx*ny*nz voxels: one scratch cube per cube (the "temporary eta" of
- * PAPER.md:430) plus a small parameter table.  0 on invalid dimensions.
+ * PAPER.md:430) plus a small parameter table and the 256-byte block holding the
+ * arrival counter of the cooperative single-launch path.  0 on invalid dimensions.
  */
 size_t idg_workspace_bytes(int nx, int ny, int nz, int batch);
 
