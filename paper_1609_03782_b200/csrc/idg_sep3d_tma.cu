@@ -6,7 +6,8 @@
 // Decomposition of the IDG kernel (idg_tma.cu): a CTA owns a 128 x (WARPS*R) xy tile and streams along z; a thread
 // owns a float4 column of an R-row strip.  Per input plane the raw tile plus RXY halo rows above and below arrives
 // by TMA (one 128 x ROWS box, zero fill outside the cube, z clamped in the plane coordinate) in a ring of NS stages:
-//   y pass  from shared memory: R + 2 RXY LDS.128 per thread, row offsets clamped to the cube once per CTA;
+//   y pass  from shared memory: R + 2 RXY LDS.128 per thread, row offsets clamped to the cube once per CTA, streamed
+//           row by row into the R accumulators (few live registers);
 //   x pass  on the y-filtered strip by warp shuffles (a radius <= 4 reaches one float4 to either side; tiles
 //           overlap by one lane on both sides; the lane just outside a cube face takes the replicated face value,
 //           which is exact because the y pass is linear and acts column by column);
@@ -132,26 +133,26 @@ idg_sep3d_tma_kernel(const __grid_constant__ SepTmaArgs S, const __grid_constant
             const float *st = stage0 + (size_t)s * G::kStageFloats;
             ptx::mbar_wait_spin(full + 8 * s, (uint32_t)((it / NS) & 1));
 
-            F4 win[WIN];
-#pragma unroll
-            for (int j = 0; j < WIN; ++j) win[j] = lds4(st + roff[j]);
-            __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(empty + 8 * s);
-
-            // y pass
+            // y pass, streamed over the window rows (row j feeds output row r with weight k = j - r): few live registers
             F4 yf[R];
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                F4 a = F4{S.wy[0] * win[r].x, S.wy[0] * win[r].y, S.wy[0] * win[r].z, S.wy[0] * win[r].w};
+            for (int j = 0; j < WIN; ++j) {
+                const F4 w = lds4(st + roff[j]);
 #pragma unroll
-                for (int k = 1; k <= 2 * RXY; ++k) {
-                    a.x = fmaf(S.wy[k], win[r + k].x, a.x);
-                    a.y = fmaf(S.wy[k], win[r + k].y, a.y);
-                    a.z = fmaf(S.wy[k], win[r + k].z, a.z);
-                    a.w = fmaf(S.wy[k], win[r + k].w, a.w);
+                for (int r = 0; r < R; ++r) {
+                    const int k = j - r;
+                    if (k == 0) {
+                        yf[r] = F4{S.wy[0] * w.x, S.wy[0] * w.y, S.wy[0] * w.z, S.wy[0] * w.w};
+                    } else if (k > 0 && k <= 2 * RXY) {
+                        yf[r].x = fmaf(S.wy[k], w.x, yf[r].x);
+                        yf[r].y = fmaf(S.wy[k], w.y, yf[r].y);
+                        yf[r].z = fmaf(S.wy[k], w.z, yf[r].z);
+                        yf[r].w = fmaf(S.wy[k], w.w, yf[r].w);
+                    }
                 }
-                yf[r] = a;
             }
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(empty + 8 * s);
             if (edge_x) {                   // replicated x faces: the lane just outside takes the face value
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
