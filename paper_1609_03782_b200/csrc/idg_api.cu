@@ -115,11 +115,20 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
             kernel = can_tile ? 2 : 1;
         }
     }
-    if (mode == 1) {          // gradient-driven variant: persistent kernel (T <= 2) or the naive kernel
-        kernel = (can_stream && g_opt[IDG_OPT_KERNEL] != 1) ? 4 : 1;
-        if (fuse > 2 || fuse == 0) fuse = 2;
-        tile = g_opt[IDG_OPT_TILE];
-        if (tile > 2 || tile == 0) tile = ((double)N * (double)batch < 6.4e7) ? 2 : 1;
+    if (mode == 1) {          // gradient-driven variant: kernel 3 (any T), the persistent kernel (option 4, T <= 2) or the naive kernel
+        const int ko = g_opt[IDG_OPT_KERNEL];
+        fuse = g_opt[IDG_OPT_FUSE];
+        if ((ko == 0 || ko == 3) && can_tma) {
+            kernel = 3;
+            if (!fuse) fuse = (nz < 100 && (double)N * (double)batch >= 4.0e6) ? 2 : 4;
+        } else if (ko != 1 && can_stream) {
+            kernel = 4;
+            if (fuse > 2 || fuse == 0) fuse = 2;
+            tile = g_opt[IDG_OPT_TILE];
+            if (tile > 2 || tile == 0) tile = ((double)N * (double)batch < 6.4e7) ? 2 : 1;
+        } else {
+            kernel = 1;
+        }
     }
     if (kernel == 4 && !can_stream) kernel = 2;
     if (kernel == 3 && !can_tma) kernel = 2;

@@ -47,6 +47,7 @@ __device__ __forceinline__ void sts4(float *p, const F4 &a)
 struct Consts {
     float2 w, ax, ay, az, s, one;
 };
+template <bool PM = false>
 __device__ __forceinline__ Consts make_consts(const CubeParams &p)
 {
     Consts k;
@@ -54,7 +55,7 @@ __device__ __forceinline__ Consts make_consts(const CubeParams &p)
     k.ax = make_float2(p.ax, p.ax);
     k.ay = make_float2(p.ay, p.ay);
     k.az = make_float2(p.az, p.az);
-    k.s = make_float2(p.s, p.s);
+    k.s = PM ? make_float2(0.25f * p.s * p.s, 0.25f * p.s * p.s) : make_float2(p.s, p.s);
     k.one = make_float2(1.0f, 1.0f);
     return k;
 }
@@ -69,9 +70,33 @@ __device__ __forceinline__ float2 update2(float2 c, float2 sx, float2 ym, float2
     const float2 r = make_float2(rcp_approx(den.x), rcp_approx(den.y));
     return __ffma2_rn(lap, r, c);
 }
+// Gradient-driven variant (Eq. 5; readings P1-P3): conductance 1/(1 + q G), G = sum_j
+// (I_{+j} - I_{-j})^2, q = s^2/4 (kept in k.s); same operation order as update_pm() of idg_kernels.cuh.
+__device__ __forceinline__ float2 update2_pm(float2 c, float2 sx, float2 gx, float2 ym, float2 yp, float2 zm,
+                                             float2 zp, const Consts &k)
+{
+    const float2 neg = make_float2(-1.0f, -1.0f);
+    const float2 lap = __ffma2_rn(k.ax, sx, __ffma2_rn(k.ay, __fadd2_rn(yp, ym),
+                                                        __ffma2_rn(k.az, __fadd2_rn(zp, zm), __fmul2_rn(k.w, c))));
+    const float2 gy = __ffma2_rn(neg, ym, yp), gz = __ffma2_rn(neg, zm, zp);
+    const float2 G = __ffma2_rn(gz, gz, __ffma2_rn(gy, gy, __fmul2_rn(gx, gx)));
+    const float2 den = __ffma2_rn(k.s, G, k.one);
+    const float2 r = make_float2(rcp_approx(den.x), rcp_approx(den.y));
+    return __ffma2_rn(lap, r, c);
+}
+template <bool PM = false>
 __device__ __forceinline__ F4 update4(const F4 &c, float left, float right, const F4 &ym, const F4 &yp,
                                       const F4 &zm, const F4 &zp, const Consts &k)
 {
+    if (PM) {
+        const float2 sx01 = make_float2(c.y + left, c.z + c.x), sx23 = make_float2(c.w + c.y, right + c.z);
+        const float2 gx01 = make_float2(c.y - left, c.z - c.x), gx23 = make_float2(c.w - c.y, right - c.z);
+        const float2 o01 = update2_pm(make_float2(c.x, c.y), sx01, gx01, make_float2(ym.x, ym.y), make_float2(yp.x, yp.y),
+                                      make_float2(zm.x, zm.y), make_float2(zp.x, zp.y), k);
+        const float2 o23 = update2_pm(make_float2(c.z, c.w), sx23, gx23, make_float2(ym.z, ym.w), make_float2(yp.z, yp.w),
+                                      make_float2(zm.z, zm.w), make_float2(zp.z, zp.w), k);
+        return F4{o01.x, o01.y, o23.x, o23.y};
+    }
     // x neighbour sums stay scalar: their operands straddle the register pairs
     const float2 sx01 = make_float2(c.y + left, c.z + c.x);
     const float2 sx23 = make_float2(c.w + c.y, right + c.z);
@@ -123,7 +148,7 @@ struct Smem {
 
 // ONE: the cube has at most 128 columns, so a single tile column covers a row with all 32 lanes valid and no halo
 // lanes; the x faces are replicated by patching the shuffled neighbour of the first / last float4 of the row.
-template <int TL, int R, int WARPS, int NS, int TMAX, bool ONE>
+template <int TL, int R, int WARPS, int NS, int TMAX, bool ONE, bool PM = false>
 __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restrict__ dst, const Launch &L,
                                          const TmaArgs &A, const CubeParams &prm, int b,
                                          unsigned char *smem, bool reinit = false)
@@ -199,7 +224,7 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
             if (q_first + i <= q_last) issue(q_first + i);
     }
 
-    const Consts kc = make_consts(prm);
+    const Consts kc = make_consts<PM>(prm);
     F4 ring[3][TL][R];
 #pragma unroll
     for (int a = 0; a < 3; ++a)
@@ -268,7 +293,7 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
                 }
                 const F4 &ym = (r == 0) ? up : cc[t][r - 1];
                 const F4 &yp = (r == R - 1) ? dn : cc[t][r + 1];
-                const F4 o = update4(c, left, right, ym, yp, zm[t][r], nw[t][r], kc);
+                const F4 o = update4<PM>(c, left, right, ym, yp, zm[t][r], nw[t][r], kc);
                 if (t + 1 < TL) nw[t + 1][r] = o;
                 else out[r] = o;
             }
@@ -298,7 +323,7 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
     }
 }
 
-template <int T, int R, int WARPS, int NS, int MINB, bool ONE>
+template <int T, int R, int WARPS, int NS, int MINB, bool ONE, bool PM = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 idg_tma_kernel(const __grid_constant__ Launch L, const __grid_constant__ TmaArgs A,
                const __grid_constant__ Maps M)
@@ -312,10 +337,10 @@ idg_tma_kernel(const __grid_constant__ Launch L, const __grid_constant__ TmaArgs
     if (now == 0) return;
     const size_t off = (size_t)b * (size_t)L.nx * (size_t)L.ny * (size_t)L.nz;
     const CUtensorMap *map = (src == L.scratch + off) ? &M.scratch : (src == L.out + off) ? &M.out : &M.in;
-    if (now == T) tma_body<T, R, WARPS, NS, T, ONE>(map, dst, L, A, prm, b, smem);
-    else if (T > 1 && now == 1) tma_body<1, R, WARPS, NS, T, ONE>(map, dst, L, A, prm, b, smem);
-    else if (T > 2 && now == 2) tma_body<(T > 2 ? 2 : 1), R, WARPS, NS, T, ONE>(map, dst, L, A, prm, b, smem);
-    else if (T > 3 && now == 3) tma_body<(T > 3 ? 3 : 1), R, WARPS, NS, T, ONE>(map, dst, L, A, prm, b, smem);
+    if (now == T) tma_body<T, R, WARPS, NS, T, ONE, PM>(map, dst, L, A, prm, b, smem);
+    else if (T > 1 && now == 1) tma_body<1, R, WARPS, NS, T, ONE, PM>(map, dst, L, A, prm, b, smem);
+    else if (T > 2 && now == 2) tma_body<(T > 2 ? 2 : 1), R, WARPS, NS, T, ONE, PM>(map, dst, L, A, prm, b, smem);
+    else if (T > 3 && now == 3) tma_body<(T > 3 ? 3 : 1), R, WARPS, NS, T, ONE, PM>(map, dst, L, A, prm, b, smem);
 }
 
 // Cooperative variant: all `A.rounds` launches of a plan in one, a grid barrier between rounds (the whole grid is
@@ -387,7 +412,7 @@ int sm_count()
 }
 
 // rounds > 1: cooperative launch of all rounds (COOP instantiation); the grid must be co-resident.
-template <int T, int R, int WARPS, int NS, int MINB, bool COOP = false>
+template <int T, int R, int WARPS, int NS, int MINB, bool COOP = false, bool PM = false>
 cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st, int rounds = 1, unsigned *bar = nullptr)
 {
     using S = Smem<T, R, WARPS, NS>;
@@ -406,7 +431,7 @@ cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st, int rounds 
     if (tiles > 0x7fffffffL) return cudaErrorInvalidValue;
     void (*kern)(Launch, TmaArgs, Maps);
     if constexpr (COOP) kern = one ? idg_tma_coop_kernel<T, R, WARPS, NS, MINB, true> : idg_tma_coop_kernel<T, R, WARPS, NS, MINB, false>;
-    else kern = one ? idg_tma_kernel<T, R, WARPS, NS, MINB, true> : idg_tma_kernel<T, R, WARPS, NS, MINB, false>;
+    else kern = one ? idg_tma_kernel<T, R, WARPS, NS, MINB, true, PM> : idg_tma_kernel<T, R, WARPS, NS, MINB, false, PM>;
     static bool attr_done[2] = {false, false};
     if (!attr_done[one]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::kBytes);
@@ -460,6 +485,15 @@ bool tma_supported(int nx, int ny, int nz, const void *in, const void *out, cons
 // 128x48 / 128x36 tile, 384 threads (T = 3: strips of 4 rows; T = 4: strips of 3).
 cudaError_t launch_tma(const Launch &L, int zchunk, int tile, cudaStream_t st)
 {
+    if (L.mode == 1) {          // gradient-driven variant (Eq. 5): the default tilings
+        switch (L.fuse) {
+        case 1: return launch_cfg<1, 4, 8, 4, 2, false, true>(L, zchunk, st);
+        case 2: return launch_cfg<2, 4, 8, 4, 2, false, true>(L, zchunk, st);
+        case 3: return launch_cfg<3, 4, 8, 4, 1, false, true>(L, zchunk, st);
+        case 4: return launch_cfg<4, 4, 8, 4, 1, false, true>(L, zchunk, st);
+        default: return cudaErrorInvalidValue;
+        }
+    }
     const bool small = (tile == 2);
     switch (L.fuse) {
     case 1: return small ? launch_cfg<1, 4, 8, 4, 2>(L, zchunk, st) : launch_cfg<1, 4, 16, 4, 1>(L, zchunk, st);

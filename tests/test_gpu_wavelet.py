@@ -190,3 +190,20 @@ def test_release_temporaries(B):
     freed = torch.cuda.mem_get_info()[0]
     assert freed >= held + 8 * 2 ** 20
     assert torch.equal(B.idg_wavelet_filter(a, B.WAVELET_LEGALL53, (1.0, 1.4, 1.7)), ref)
+
+
+def test_haar_warp_kernel_full_size_equals_per_axis_passes(B):
+    """configs[2] size (512 x 512 x 256), the launch configuration bench.py --filter wavelet_haar times: the
+    block-per-warp kernel against the per-level, per-axis in-place passes, bit for bit, with the paper's thresholds."""
+    g = torch.Generator(device="cuda").manual_seed(31)
+    a = torch.randn((256, 512, 512), device="cuda", generator=g)
+    a[100:110, 200:230, 300:340] += 6.0
+    B.idg_set_option(B.IDG_OPT_KERNEL, 1)
+    try:
+        ref = B.idg_wavelet_filter(a, B.WAVELET_HAAR, (0.5, 0.8, 1.1), 1.0)
+    finally:
+        B.idg_set_option(B.IDG_OPT_KERNEL, 0)
+    out = B.idg_wavelet_filter(a, B.WAVELET_HAAR, (0.5, 0.8, 1.1), 1.0)
+    assert "idg_haar_warp_kernel" in B.idg_last_plan()
+    assert torch.equal(out, ref)
+    assert int((out != a).sum()) > a.numel() // 2          # the filter did something
