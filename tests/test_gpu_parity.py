@@ -129,21 +129,48 @@ def test_stream_grid_variants(B, oracle, fuse, tile, ctas):
     assert err(gpu(B, a, 7, p), oracle.idg_filter_oracle(a, 7, **p.f32()), 2.0) <= TOL
 
 
-def test_config1_parameter_sweep(B, oracle):
-    """configs[1]: S/N 22 and 62 cubes, 8 K values, n = 1..40 (snapshots at 1, 5, 10, 20, 40 here;
-    the oracle runs incrementally -- Markov property, pinned by test_p11)."""
+def test_config1_parameter_sweep(B, oracle, parity_log):
+    """configs[1] as BASELINE.json states it: S/N 22 and 62 cubes x 8 K values x EVERY n = 1..40 = 640 outputs
+    (the paper's parameter exploration).  The oracle advances one iteration at
+    a time (Markov property, pinned by test_p11); the GPU runs each n (i) from scratch as one 16-cube batched
+    call -- the call `bench.py --workload cfg1_sweep` times -- and (ii) incrementally, one more iteration on its own
+    previous output."""
     from paper_1609_03782_b200 import synth
     set_plan(B, (0, 0))
+    cubes, ps, rms = [], [], []
     for seed, snr in ((1001, 22.0), (1002, 62.0)):
         c = synth.modelb_like(seed=seed, snr=snr)
         assert c.peak < 64.0, "fp32 rounding floor argument needs max|I| < 64 rms (DESIGN.md section 6)"
         for K in synth.K_SWEEP:
-            p = B.Params(K=K)
-            ref, done = c.data.astype(np.float64), 0
-            for n in (1, 5, 10, 20, 40):
-                ref = oracle.idg_filter_oracle(ref, n - done, **p.f32())
-                done = n
-                assert err(gpu(B, c.data, n, p), ref, c.rms) <= TOL, (snr, K, n)
+            cubes.append(c.data)
+            ps.append(B.Params(K=K))
+            rms.append(c.rms)
+    nb = len(cubes)
+    assert nb == 16
+    t = torch.from_numpy(np.stack(cubes)).cuda()
+    ws = B.alloc_workspace(100, 100, 67, nb)
+    refs = [c.astype(np.float64) for c in cubes]
+    inc = t.clone()
+    worst_scratch = worst_inc = 0.0
+    for n in range(1, 41):
+        refs = [oracle.idg_filter_oracle(r, 1, **p.f32()) for r, p in zip(refs, ps)]
+        scratch = B.idg_filter_batched(t, n, ps, workspace=ws)
+        inc = B.idg_filter_batched(inc, 1, ps, workspace=ws)
+        torch.cuda.synchronize()
+        sc, ic = scratch.cpu().numpy(), inc.cpu().numpy()
+        for b in range(nb):
+            e1, e2 = err(sc[b], refs[b], rms[b]), err(ic[b], refs[b], rms[b])
+            assert e1 <= TOL and e2 <= TOL, (b, ps[b].K, n, e1, e2)
+            worst_scratch, worst_inc = max(worst_scratch, e1), max(worst_inc, e2)
+    parity_log("cfg1 2x8x40 from scratch (16-cube batches)", worst_scratch, "640 outputs, full cubes")
+    parity_log("cfg1 2x8x40 incremental", worst_inc, "640 outputs, full cubes")
+    # single-cube calls (the cooperative / resident small-cube plans) on a subset of the sweep
+    for b in (0, 8, 15):
+        ref = cubes[b].astype(np.float64)
+        for n in range(1, 41):
+            ref = oracle.idg_filter_oracle(ref, 1, **ps[b].f32())
+            if n in (1, 2, 3, 4, 5, 7, 10, 13, 20, 31, 40):
+                assert err(gpu(B, cubes[b], n, ps[b]), ref, rms[b]) <= TOL, (b, n)
 
 
 def test_incremental_equals_from_scratch(B):
@@ -187,27 +214,40 @@ def check_blocks(oracle, cube, out, n, p, blocks, rms):
     return worst
 
 
-def test_config2_survey_field(B, oracle):
-    """configs[2]: 512x512x256, 6 discs, defaults, n = 20; 40 sub-blocks incl. all corners, plus
-    the block around the brightest voxel."""
+def full_cube_err(oracle, cube, out, n, p, rms):
+    """max |gpu - oracle| / rms over the WHOLE cube (OpenMP oracle, fp64 buffers: 3 x 8 B per voxel of host memory)."""
+    ref = oracle.idg_filter_oracle(cube, n, **p.f32())
+    worst = 0.0
+    for z in range(0, cube.shape[0], 32):            # in slabs: no fourth cube-sized temporary
+        worst = max(worst, float(np.abs(out[z:z + 32].astype(np.float64) - ref[z:z + 32]).max()))
+    return worst / rms
+
+
+def host_has(gib: float) -> bool:
+    try:
+        import psutil
+        return psutil.virtual_memory().available >= gib * 2 ** 30
+    except Exception:
+        return False
+
+
+def test_config2_survey_field(B, oracle, parity_log):
+    """configs[2]: 512x512x256, 6 discs, defaults, n = 20; the whole cube against the OpenMP oracle."""
     from paper_1609_03782_b200 import synth
     set_plan(B, (0, 0))
     c = synth.survey_field((256, 512, 512), seed=2000, n_discs=6)
     p = B.Params()
     out = gpu(B, c.data, 20, p)
-    rng = np.random.default_rng(2)
-    blocks = sub_blocks(c.data.shape, 20, 24, 40, rng)
-    bz, by, bx = np.unravel_index(np.argmax(c.data), c.data.shape)
-    blocks.append((max(bz - 32, 0), min(bz + 32, 256), max(by - 32, 0), min(by + 32, 512),
-                   max(bx - 32, 0), min(bx + 32, 512)))
-    assert check_blocks(oracle, c.data, out, 20, p, blocks, c.rms) <= TOL
+    e = full_cube_err(oracle, c.data, out, 20, p, c.rms)
+    parity_log("cfg2 512x512x256 n=20", e, "full cube, " + B.idg_last_plan())
+    assert e <= TOL
 
 
-def test_config3_large_cube(B, oracle):
-    """configs[3]: 1024x1024x512 (2.1 GB), 20 discs + extra-planar gas, defaults, n = 20, in the
-    launch configuration bench.py times (auto plan, workspace variant).  The oracle cannot hold
-    the full cube in seconds, so 48 sub-blocks (all 8 corners, faces, random interior, brightest
-    voxel) are compared on their exact inner region."""
+def test_config3_large_cube(B, oracle, parity_log):
+    """configs[3]: 1024x1024x512 (2.1 GB), 20 discs + extra-planar gas, defaults, n = 20, in the launch configuration
+    bench.py times (auto plan, workspace variant): the WHOLE cube against the OpenMP oracle (3 x 4.3 GB of fp64
+    buffers, ~5 s on 16 cores).  Only when the host has less than 24 GB free: 48 sub-blocks (all 8 corners, faces,
+    random interior, brightest voxel) compared on their exact inner region; the parity log says which ran."""
     from paper_1609_03782_b200 import synth
     free, _ = torch.cuda.mem_get_info()
     if free < 8 * 2 ** 30:
@@ -219,34 +259,76 @@ def test_config3_large_cube(B, oracle):
     ws = B.alloc_workspace(1024, 1024, 512, 1)
     o = B.idg_filter(t, 20, p, workspace=ws)
     torch.cuda.synchronize()
+    plan = B.idg_last_plan()
     out = o.cpu().numpy()
-    rng = np.random.default_rng(3)
-    blocks = sub_blocks(c.data.shape, 20, 24, 47, rng)
-    bz, by, bx = np.unravel_index(np.argmax(c.data), c.data.shape)
-    blocks.append((max(bz - 32, 0), min(bz + 32, 512), max(by - 32, 0), min(by + 32, 1024),
-                   max(bx - 32, 0), min(bx + 32, 1024)))
-    assert check_blocks(oracle, c.data, out, 20, p, blocks, c.rms) <= TOL
+    del t, o, ws
     assert np.isfinite(out).all()
+    if host_has(24.0):
+        e = full_cube_err(oracle, c.data, out, 20, p, c.rms)
+        parity_log("cfg3 1024x1024x512 n=20", e, "full cube, " + plan)
+    else:
+        rng = np.random.default_rng(3)
+        blocks = sub_blocks(c.data.shape, 20, 24, 47, rng)
+        bz, by, bx = np.unravel_index(np.argmax(c.data), c.data.shape)
+        blocks.append((max(bz - 32, 0), min(bz + 32, 512), max(by - 32, 0), min(by + 32, 1024),
+                       max(bx - 32, 0), min(bx + 32, 1024)))
+        e = check_blocks(oracle, c.data, out, 20, p, blocks, c.rms)
+        parity_log("cfg3 1024x1024x512 n=20", e, "48 SUB-BLOCKS ONLY (host memory < 24 GB), " + plan)
+    assert e <= TOL
 
 
-def test_config4_batched(B, oracle):
-    """configs[4]: 128x128x64 cubes with per-cube parameters, n = 10, one batched call.
-    32 cubes against the oracle; all of them against single-cube calls bitwise."""
+def test_config4_batched(B, oracle, parity_log):
+    """configs[4] as BASELINE.json states it: 256 cubes of 128x128x64 with per-cube parameters, n = 10, in ONE batched
+    call (grid z = 256, 1.07 GB: the launch bench.py --workload cfg4... times).  All 256 cubes against the oracle, and
+    all of them against single-cube calls bitwise."""
     from paper_1609_03782_b200 import synth
     set_plan(B, (0, 0))
-    nb = 32
+    nb = 256
     cubes = synth.batch_cubes(nb, seed=4000)
-    prm = synth.batch_params(256, seed=4000)[:nb]
+    prm = synth.batch_params(nb, seed=4000)
     ps = [B.Params(*[float(v) for v in row]) for row in prm]
     t = torch.from_numpy(cubes).cuda()
-    out = B.idg_filter_batched(t, 10, ps)
+    ws = B.alloc_workspace(128, 128, 64, nb)
+    out = B.idg_filter_batched(t, 10, ps, workspace=ws)
+    plan = B.idg_last_plan()
     torch.cuda.synchronize()
     o = out.cpu().numpy()
+    worst = 0.0
     for b in range(nb):
         ref = oracle.idg_filter_oracle(cubes[b], 10, **ps[b].f32())
-        assert err(o[b], ref, 1.0) <= TOL, b
+        e = err(o[b], ref, 1.0)
+        assert e <= TOL, (b, e)
+        worst = max(worst, e)
         single = B.idg_filter(t[b], 10, ps[b])
         assert torch.equal(single, out[b]), b
+    parity_log("cfg4 256 x 128x128x64 n=10, one call", worst, "all 256 cubes, " + plan)
+
+
+def test_bright_plateau_expanded_numerator(B, oracle, parity_log):
+    """DESIGN.md reading R14: the kernels evaluate the numerator of Eq. 7 in expanded form, a_j (p_j + m_j) + w c,
+    which is not exactly stationary on a plateau as the paper's difference form is.  Worst case: a slab
+    at 500 rms with noise, n = 40, K = 10 and K = +inf (no S ~ K^2/I^2 damping of the rounding error).  At 500 rms
+    one fp32 ulp is 2^-15 = 3.05e-5 rms, so the 1e-4 x rms bar is out of reach of ANY fp32 form there; the bar on the
+    slab is the arithmetic's own bound per iteration, ulp/2 for the final add plus 4 ulp x S for the cancellation
+    inside the numerator (|a_j (p + m)| ~ |w c| ~ 488), times n (the scheme is contractive: errors do not grow).
+    More than n voxels away from the slab (exact domain of dependence, pin P8) the 1e-4 bar holds as everywhere."""
+    rng = np.random.default_rng(41)
+    a = rng.normal(0, 1, (24, 40, 160)).astype(np.float32)
+    a[6:18, 8:32, 12:52] += 500.0
+    ulp, n = 2.0 ** -15, 40
+    for K in (10.0, math.inf):
+        S = 0.0 if math.isinf(K) else 1.0 / (1.0 + 500.0 ** 2 / K ** 2)
+        bar = n * ulp * (0.5 + 4.0 * (1.0 if math.isinf(K) else S))
+        p = B.Params(K=K)
+        ref = oracle.idg_filter_oracle(a, n, **p.f32())
+        for plan in ((1, 0), (3, 4), (0, 0)):
+            set_plan(B, plan)
+            out = gpu(B, a, n, p)
+            e = err(out, ref, 1.0)
+            parity_log(f"bright plateau 500 rms K={K} n=40 plan={plan[0]},{plan[1]}", e,
+                       f"bar on the slab {bar:.1e} = n ulp(500) (1/2 + 4 S); faint part: 1e-4")
+            assert e <= bar, (K, plan, e)
+            assert err(out[:, :, 100:], ref[:, :, 100:], 1.0) <= TOL
 
 
 def test_batched_mixed_iteration_counts(B, oracle):
