@@ -18,7 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libidg_b200.so")
 
 IDG_OPT_KERNEL, IDG_OPT_FUSE, IDG_OPT_ZCHUNK, IDG_OPT_TILE, IDG_OPT_CTAS, IDG_OPT_HOST_SLABS, IDG_OPT_COOP = 0, 1, 2, 3, 4, 5, 6
-KERNEL_AUTO, KERNEL_NAIVE, KERNEL_TILED, KERNEL_TMA, KERNEL_STREAM = 0, 1, 2, 3, 4
+KERNEL_AUTO, KERNEL_NAIVE, KERNEL_TILED, KERNEL_TMA, KERNEL_STREAM, KERNEL_RESIDENT = 0, 1, 2, 3, 4, 5
 
 # every symbol include/idg.h declares (tests check the library exports them all)
 SYMBOLS = ("idg_version", "idg_status_string", "idg_params_check", "idg_workspace_bytes",

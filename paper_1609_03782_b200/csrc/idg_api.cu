@@ -31,6 +31,10 @@ bool voxel_count(int nx, int ny, int nz, int batch, size_t *n_one)
     return true;
 }
 
+// Shapes the resident kernel can take (float4 rows, a cube small enough to sit in the SMs' shared memory): the
+// workspace then carries the mailbox region.
+bool resident_shape(int nx, size_t N) { return nx % 4 == 0 && N <= idg::kResidentMaxCubeVoxels; }
+
 bool params_valid(const idg_params &p)
 {
     if (!(p.K > 0.0f)) return false;                         // rejects NaN, 0, negatives; +inf passes
@@ -88,6 +92,8 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     float *scratch = (float *)workspace;
     idg::CubeParams *tab = (idg::CubeParams *)((char *)workspace + align_up(bytes));
     unsigned *coop_bar = (unsigned *)((char *)tab + align_up(sizeof(idg::CubeParams) * (size_t)batch));
+    unsigned long long *mail = (unsigned long long *)((char *)coop_bar + kAlign);
+    const size_t mail_bytes = resident_shape(nx, N) ? idg::kResidentMailBytes : 0;
 
     // Plan: kernel variant and iterations fused per launch.
     const bool can_tile = idg::tiled_supported(nx, ny, nz, cubes, out, scratch);
@@ -96,6 +102,14 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     int kernel = g_opt[IDG_OPT_KERNEL];
     int fuse = g_opt[IDG_OPT_FUSE];
     int tile = g_opt[IDG_OPT_TILE];
+    // Small cubes and interactive batches: everything on chip for the whole call (profiles/r2a_notes.md).
+    idg::ResidentPlan rplan;
+    const bool can_resident = mail_bytes > 0 && max_n > 0 && (((uintptr_t)cubes | (uintptr_t)out) & 15u) == 0 &&
+                              (kernel == 0 || kernel == 5) &&
+                              idg::resident_plan(nx, ny, nz, batch, max_n, mail_bytes, idg::device_sm_count(), &rplan);
+    if (kernel == 5 && !can_resident) kernel = 0;
+    // Measured (profiles/r2a_notes.md): faster than kernel 3 when the whole call fits on chip at once (one wave).
+    if (kernel == 0 && can_resident && fuse == 0 && rplan.cubes >= batch) kernel = 5;
     if (kernel == 0) {
         // Measured on B200 (profiles/r1g_notes.md, r1h_notes.md): the z-chunked TMA kernel everywhere it applies.
         // Four fused iterations per launch (one 8-warp CTA per SM) move a quarter of the DRAM bytes of an un-fused
@@ -115,7 +129,7 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
             kernel = can_tile ? 2 : 1;
         }
     }
-    if (mode == 1) {          // gradient-driven variant: kernel 3 (any T), the persistent kernel (option 4, T <= 2) or the naive kernel
+    if (mode == 1 && kernel != 5) {          // gradient-driven variant: kernel 3 (any T), the persistent kernel (option 4, T <= 2) or the naive kernel
         const int ko = g_opt[IDG_OPT_KERNEL];
         fuse = g_opt[IDG_OPT_FUSE];
         if ((ko == 0 || ko == 3) && can_tma) {
@@ -133,15 +147,17 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     if (kernel == 4 && !can_stream) kernel = 2;
     if (kernel == 3 && !can_tma) kernel = 2;
     if (kernel == 2 && !can_tile) kernel = 1;
-    if (kernel >= 2) {
+    if (kernel == 5) {
+        fuse = max_n;
+    } else if (kernel >= 2) {
         if (!fuse) fuse = 2;
         if (fuse > max_n && max_n > 0) fuse = max_n;
     } else {
         fuse = 1;
     }
     {
-        static const char *const names[5] = {"", "idg_naive_kernel", "idg_tiled_kernel", "idg_tma_kernel",
-                                             "idg_stream_kernel"};
+        static const char *const names[6] = {"", "idg_naive_kernel", "idg_tiled_kernel", "idg_tma_kernel",
+                                             "idg_stream_kernel", "idg_resident_kernel"};
         snprintf(t_plan, sizeof(t_plan), "%s%s fuse=%d tile=%d", names[kernel], mode == 1 ? " pm" : "", fuse, tile);
     }
 
@@ -187,6 +203,17 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
                             cudaMemcpyHostToDevice, st);
         if (e != cudaSuccess) return (int)e;
         L.tab = tab;
+    }
+    if (kernel == 5) {  // one cooperative launch per wave of cubes; reads `cubes` once, writes `out` once (in place is safe)
+        int launches = 0;
+        e = idg::launch_resident(L, rplan, mail, st, &launches);
+        if (e == cudaSuccess) {
+            t_launches = launches;
+            snprintf(t_plan, sizeof(t_plan), "idg_resident_kernel%s blocks=%dx%d of %dx%dx%d waves=%d", mode == 1 ? " pm" : "",
+                     rplan.ty, rplan.tz, nx, rplan.by, rplan.bz, launches);
+            return IDG_OK;
+        }
+        return (int)e;
     }
     if (in_place) {     // stage I_0 so a cube whose first launch targets `out` does not read what it writes
         e = cudaMemcpyAsync(scratch, cubes, bytes, cudaMemcpyDeviceToDevice, st);
@@ -268,7 +295,8 @@ size_t idg_workspace_bytes(int nx, int ny, int nz, int batch)
     size_t N;
     if (!voxel_count(nx, ny, nz, batch, &N)) return 0;
     return align_up(N * (size_t)batch * sizeof(float)) + align_up(sizeof(idg::CubeParams) * (size_t)batch) +
-           kAlign;      // scratch cubes | per-cube constants | arrival counter of the cooperative launch
+           kAlign +     // scratch cubes | per-cube constants | arrival counter of the cooperative launch
+           (resident_shape(nx, N) ? idg::kResidentMailBytes : 0);      // | mailboxes of the resident kernel
 }
 
 int idg_filter_ws(const float *cube, int nx, int ny, int nz, int n_iter, const idg_params *params,
@@ -748,7 +776,7 @@ int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, i
 int idg_set_option(int key, int value)
 {
     if (key < 0 || key >= IDG_OPT_COUNT_) return IDG_ERR_OPTION;
-    if (key == IDG_OPT_KERNEL && (value < 0 || value > 4)) return IDG_ERR_OPTION;
+    if (key == IDG_OPT_KERNEL && (value < 0 || value > 5)) return IDG_ERR_OPTION;
     if (key == IDG_OPT_FUSE && (value < 0 || value > 4)) return IDG_ERR_OPTION;
     if (key == IDG_OPT_ZCHUNK && value < 0) return IDG_ERR_OPTION;
     if (key == IDG_OPT_TILE && (value < 0 || value > 4)) return IDG_ERR_OPTION;

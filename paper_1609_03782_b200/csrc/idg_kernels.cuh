@@ -113,6 +113,23 @@ bool tma_supported(int nx, int ny, int nz, const void *in, const void *out, cons
 cudaError_t launch_stream(const Launch &L, int nctas, int tile, cudaStream_t st);
 bool stream_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
 
+// Resident kernel (idg_resident.cu): the cube(s) stay in shared memory for all iterations of a call; block faces are
+// exchanged through mailboxes in the workspace.  resident_plan() picks the block decomposition (false: the shape does
+// not fit); launch_resident() enqueues one cooperative launch per wave of cubes.
+struct ResidentPlan {
+    int ty, tz;             // blocks per cube along y, z
+    int by, bz;             // nominal block extents
+    int ls;                 // z cells per warp work item
+    int cubes;              // cubes per launch (wave)
+    int words;              // 64-bit mailbox words per (block, parity)
+    size_t smem;            // dynamic shared memory per CTA
+};
+constexpr size_t kResidentMailBytes = (size_t)32 << 20;       // mailbox region reserved in the workspace
+constexpr size_t kResidentMaxCubeVoxels = (size_t)4 << 20;     // larger cubes cannot be held on chip
+bool resident_plan(int nx, int ny, int nz, int batch, int max_n, size_t mail_bytes, int sms, ResidentPlan *out);
+cudaError_t launch_resident(const Launch &L, const ResidentPlan &P, unsigned long long *mail, cudaStream_t st,
+                            int *launches);
+int device_sm_count();      // SMs of the current device (148 when it cannot be queried)
 
 // Stream-ordered temporaries (idg_tmap.cu): cudaMallocAsync from a private memory pool that keeps what it has
 // been given (release threshold = everything), so a call that needs a cube-sized temporary does not pay the

@@ -29,9 +29,9 @@ def B():
 
 # (kernel, fuse) plans every parity case runs under
 PLANS = [(1, 0), (2, 1), (2, 2), (2, 3), (2, 4), (3, 1), (3, 2), (3, 3), (3, 4),
-         (4, 1), (4, 2), (4, 3), (4, 4), (0, 0)]
+         (4, 1), (4, 2), (4, 3), (4, 4), (5, 0), (0, 0)]
 PLAN_IDS = ["naive", "tiled-T1", "tiled-T2", "tiled-T3", "tiled-T4", "tma-T1", "tma-T2", "tma-T3", "tma-T4",
-            "stream-T1", "stream-T2", "stream-T3", "stream-T4", "auto"]
+            "stream-T1", "stream-T2", "stream-T3", "stream-T4", "resident", "auto"]
 
 
 def set_plan(B, plan, zchunk=0, tile=0, ctas=0, coop=None):
@@ -510,14 +510,52 @@ def test_cooperative_launch_batched_mixed_iteration_counts(B, oracle):
         assert torch.equal(out[b], B.idg_filter(xs[b], ns[b], ps[b])), b
 
 
-def test_auto_plan_uses_the_cooperative_launch_for_small_cubes_only(B):
+def test_auto_plan_by_size(B):
+    """Auto plan: the resident kernel (cube on chip for the whole call, one cooperative launch) when the whole call fits
+    on chip at once; kernel 3 for larger cubes and batches; option COOP = 2 still folds kernel 3's rounds."""
     set_plan(B, (0, 0))
     B.idg_filter(torch.zeros(67, 100, 100, device="cuda"), 10)
-    assert "idg_tma_coop_kernel" in B.idg_last_plan() and B.idg_last_launch_count() == 1
+    assert "idg_resident_kernel" in B.idg_last_plan() and B.idg_last_launch_count() == 1
     B.idg_filter(torch.zeros(128, 512, 512, device="cuda"), 8)
     assert "idg_tma_kernel" in B.idg_last_plan() and B.idg_last_launch_count() == 2
-    B.idg_filter(torch.zeros(8, 16, 16, device="cuda"), 3)          # one round: nothing to fold
+    B.idg_filter_batched(torch.zeros(16, 67, 100, 100, device="cuda"), 10, [B.Params()] * 16)
     assert "idg_tma_kernel" in B.idg_last_plan()
+    B.idg_filter(torch.zeros(8, 16, 18, device="cuda"), 3)           # nx % 4 != 0
+    assert "idg_resident_kernel" not in B.idg_last_plan()
+    set_plan(B, (3, 3), coop=2)
+    B.idg_filter(torch.zeros(67, 100, 100, device="cuda"), 10)
+    assert "idg_tma_coop_kernel" in B.idg_last_plan() and B.idg_last_launch_count() == 1
+
+
+@pytest.mark.parametrize("shape,nb", [((67, 100, 100), 1), ((5, 9, 8), 1), ((1, 1, 8), 1), ((3, 300, 16), 1), ((200, 3, 24), 1),
+                                      ((64, 128, 128), 3), ((67, 100, 100), 7), ((20, 24, 520), 2), ((128, 128, 128), 1),
+                                      ((33, 77, 132), 5)],
+                         ids=lambda v: "x".join(map(str, v[::-1])) if isinstance(v, tuple) else f"b{v}")
+def test_resident_kernel_is_bitwise_equal_to_the_naive_kernel_and_repeatable(B, shape, nb):
+    """idg_resident_kernel: blocks of the cube stay in shared memory for all iterations, faces travel through mailboxes
+    with the iteration tag packed into every word.  Same arithmetic as every other kernel -> bit-identical to the
+    one-thread-per-voxel kernel, on every run (a face read before it arrived, or a mailbox overwritten too early, would
+    show as a differing voxel), for ragged blocks, one to several waves of cubes, per-cube iteration counts (0 included),
+    in place, and for the gradient-driven variant."""
+    g = torch.Generator(device="cuda").manual_seed(5)
+    x = torch.randn((nb,) + shape, device="cuda", generator=g) * 2.0
+    ps = [B.Params(K=1.0 + 0.25 * b, tau=0.03, cx=5.0, cy=4.0, cz=6.0, rms=1.0) for b in range(nb)]
+    for ns in ([1] * nb, [2] * nb, [(3 * b + 7) % 12 for b in range(nb)], [40] * nb):
+        set_plan(B, (1, 0))
+        ref = B.idg_filter_batched(x, ns, ps)
+        for rep in range(3):
+            set_plan(B, (5, 0))
+            out = B.idg_filter_batched(x, ns, ps)
+            torch.cuda.synchronize()
+            assert "idg_resident_kernel" in B.idg_last_plan(), B.idg_last_plan()
+            assert torch.equal(out, ref), (shape, nb, ns, rep, int((out != ref).sum()))
+        inplace = x.clone()
+        B.idg_filter_batched(inplace, ns, ps, out=inplace)
+        assert torch.equal(inplace, ref)
+    set_plan(B, (1, 0))
+    ref = B.idg_filter_pm(x[0], 5, ps[0])
+    set_plan(B, (5, 0))
+    assert torch.equal(B.idg_filter_pm(x[0], 5, ps[0]), ref) and "idg_resident_kernel pm" in B.idg_last_plan()
 
 
 @pytest.mark.parametrize("plan", [(2, 2), (3, 1), (3, 2), (3, 3), (3, 4), (4, 1), (4, 2), (4, 3), (4, 4)],
