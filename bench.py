@@ -37,8 +37,12 @@ WORKLOADS = {
     "cfg2_512x512x256_n20": ((256, 512, 512), 20, "survey"),
     "cfg0_100x100x67_n10": ((67, 100, 100), 10, "modelb"),
     "cfg4_256x128x128x64_n10": ((64, 128, 128), 10, "batch"),      # 256 cubes, per-cube parameters
+    # configs[1]: S/N 22 and 62 cubes x 8 K values; a step = the whole exploration, one batched 16-cube call per n = 1..40
+    "cfg1_sweep_2x8x40": ((67, 100, 100), 40, "sweep"),
 }
 BATCH = 256
+L2_BYTES = 126e6                    # B200 L2 (B200_PROFILING.md)
+L2_PEAK_GBS = 6300 * 1.965          # ~6300 B/clk chip-wide LTS cap x 1.965 GHz (B300_MICROARCH.md, L2 cache) = 12.4 TB/s
 # reference filters (PAPER.md:402-405 timing parameters); --filter idg is the contract's metric
 FILTERS = {"idg": None, "box": ("box", (3, 3, 3)), "box_aniso": ("box", (3, 5, 5)),
            "gauss": ("gauss", (3.0, 3.0, 3.0), (0.0, 0.0, 0.0)), "gauss_aniso": ("gauss", (2.0, 3.0, 3.0), (0.0, 0.0, 0.0)),
@@ -71,17 +75,28 @@ def measured_peak_gbs():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic_bytes(kernel_tag: str):
-    """dram read+write bytes per launch of the dominant kernel from the committed ncu summary."""
-    p = os.path.join(ROOT, "profiles", "traffic.txt")
+def ncu_counters(plan: str, workload: str) -> dict:
+    """Per-launch ncu counters of the dominant kernel of (plan, workload) from the committed table
+    profiles/ncu_per_launch.json (each entry names its source note and commit); {} when this plan on this workload
+    has never been captured -- then the line carries no traffic figure rather than someone else's."""
     try:
-        for line in open(p):
-            k, _, v = line.partition(" = ")              # the key itself holds '=' signs ("fuse=4")
-            if k.strip() == kernel_tag:
-                return float(v.split()[0])
+        with open(os.path.join(ROOT, "profiles", "ncu_per_launch.json")) as f:
+            for e in json.load(f)["entries"]:
+                if e["plan"] == plan and e["workload"] == workload:
+                    return e
     except Exception:
         pass
-    return None
+    return {}
+
+
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
 
 
 class ClockSampler:
@@ -132,10 +147,10 @@ class ClockSampler:
                 "sm_max_mhz": max(mx) if mx else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_rate(cube: np.ndarray, n_iter: int, target_s: float, prm: dict):
+def oracle_rate(cube: np.ndarray, n_iter: int, target_s: float, prm: dict, threads=None):
     """Time the oracle, as it stands, on a bounded sample: the first planes of the workload cube."""
     import oracle
-    cores = oracle.set_threads(os.cpu_count() or 1)
+    cores = oracle.set_threads(threads or os.cpu_count() or 1)
     nz, ny, nx = cube.shape
     probe = cube[: min(nz, 4)]
     t0 = time.perf_counter()
@@ -187,7 +202,8 @@ def run_reference(args) -> None:
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": args.workload, "n_iter": n, "params": "K=1.5 tau=0.0325 C=5 (PAPER.md:187)",
                    "sample": desc},
-        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                         "cpu_model": cpu_model()},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
@@ -213,6 +229,7 @@ def run_ours(args) -> None:
     import torch
     import torch.distributed as dist
     from paper_1609_03782_b200 import binding as B
+    from paper_1609_03782_b200 import synth
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -223,46 +240,56 @@ def run_ours(args) -> None:
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     B.lib()                                   # fail loudly if the extension is missing
+    B.idg_set_option(B.IDG_OPT_KERNEL, args.kernel)
     B.idg_set_option(B.IDG_OPT_FUSE, args.fuse)
     B.idg_set_option(B.IDG_OPT_ZCHUNK, args.zchunk)
     B.idg_set_option(B.IDG_OPT_TILE, args.tile)
 
     threads = max(1, (os.cpu_count() or 1) // max(1, world))
-    batched = WORKLOADS[args.workload][2] == "batch"
+    shape, n, gen = WORKLOADS[args.workload]
+    batched, sweep = gen == "batch", gen == "sweep"
     filt = FILTERS[args.filter]
+    nz, ny, nx = shape
+    nb = 1
     if batched:
-        from paper_1609_03782_b200 import synth
-        shape, n, _ = WORKLOADS[args.workload]
-        data = synth.batch_cubes(BATCH, seed=4000 + 1000 * rank, shape=shape, threads=threads)
-        plist = [B.Params(*[float(v) for v in row]) for row in synth.batch_params(BATCH, seed=4000 + 1000 * rank)]
-        nz, ny, nx = shape
-        N = BATCH * nz * ny * nx
-        args.no_e2e = True                    # the host-buffer entry point takes one cube
+        nb = BATCH
+        data = synth.batch_cubes(nb, seed=4000 + 1000 * rank, shape=shape, threads=threads)
+        plist = [B.Params(*[float(v) for v in row]) for row in synth.batch_params(nb, seed=4000 + 1000 * rank)]
+    elif sweep:                               # configs[1]: 2 cubes x 8 K
+        two = [synth.modelb_like(shape, seed=1001 + 10 * rank, snr=22.0, threads=threads).data,
+               synth.modelb_like(shape, seed=1002 + 10 * rank, snr=62.0, threads=threads).data]
+        data = np.stack([two[i] for i in (0, 1) for _ in synth.K_SWEEP])
+        plist = [B.Params(K=float(K)) for _ in (0, 1) for K in synth.K_SWEEP]
+        nb = len(plist)
     else:
         cube, n = make_cube(args.workload, seed_offset=rank, threads=threads)
         data = cube.data
-        nz, ny, nx = data.shape
-        N = nz * ny * nx
+    N = nb * nz * ny * nx
+    if nb > 1:
+        args.no_e2e = True                    # the host-buffer entry point takes one cube
     p = B.Params()                            # PAPER.md:187 defaults; rms = 1 by construction
     host_in = torch.from_numpy(data).pin_memory()
     d_in = host_in.cuda(non_blocking=True)
     d_out = torch.empty_like(d_in)
-    ws = B.alloc_workspace(nx, ny, nz, BATCH if batched else 1)
+    ws = B.alloc_workspace(nx, ny, nz, nb)
     stream = torch.cuda.current_stream()
     if filt is not None:
-        if batched:
+        if nb > 1:
             raise SystemExit("--filter box/gauss runs on single-cube workloads")
         n = 1                                 # one pass; throughput in Gvoxel/s
         args.no_e2e = True
         if filt[0] == "quality":              # the "filtered" cube: a box-smoothed copy
             B.idg_box_filter(d_in, 3, 3, 3, out=d_out, stream=stream)
             q_sums = torch.empty(8, dtype=torch.float64, device="cuda")
+    voxel_iters = N * (n * (n + 1) // 2 if sweep else n)      # per step
 
     def barrier():
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    launches = [0]
 
     def step():
         if filt is not None:
@@ -274,33 +301,85 @@ def run_ours(args) -> None:
                 B.idg_box_filter(d_in, *filt[1], out=d_out, stream=stream)
             else:
                 B.idg_gaussian_filter(d_in, filt[1], filt[2], out=d_out, stream=stream)
+            launches[0] = B.idg_last_launch_count()
+        elif sweep:                           # every n from scratch, one batched call each
+            launches[0] = 0
+            for k in range(1, n + 1):
+                B.idg_filter_batched(d_in, k, plist, out=d_out, workspace=ws, stream=stream)
+                launches[0] += B.idg_last_launch_count()
         elif batched:
             B.idg_filter_batched(d_in, n, plist, out=d_out, workspace=ws, stream=stream)
+            launches[0] = B.idg_last_launch_count()
         else:
             B.idg_filter(d_in, n, p, out=d_out, workspace=ws, stream=stream)
+            launches[0] = B.idg_last_launch_count()
 
-    for _ in range(max(3, args.warmup)):
+    warm = max(3, args.warmup)
+    for _ in range(warm):
         step()
-    launches_per_step = B.idg_last_launch_count()
+    launches_per_step = launches[0]
     plan = B.idg_last_plan()
-    fuse = -(-n // launches_per_step)
+    fuse = max(1, -(-n // launches_per_step)) if not sweep else 1
     barrier()
+
+    # L2 rule: a working set (input + output of a call) that fits the 126 MB L2 is timed COLD -- a 512 MB scratch
+    # write between the timed calls, outside the events -- and the back-to-back (warm) figure is reported beside it.
+    fits_l2 = 2 * N * 4 <= 2 * L2_BYTES
+    flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device="cuda") if fits_l2 else None
+
+    def timed(steps: int, flush: bool) -> float:
+        e0 = [torch.cuda.Event(enable_timing=True) for _ in range(steps if flush else 1)]
+        e1 = [torch.cuda.Event(enable_timing=True) for _ in range(steps if flush else 1)]
+        if not flush:
+            e0[0].record(stream)
+            for _ in range(steps):
+                step()
+            e1[0].record(stream)
+        else:
+            for i in range(steps):
+                flush_buf.fill_(i & 0xff)
+                e0[i].record(stream)
+                step()
+                e1[i].record(stream)
+        barrier()
+        return sum(a.elapsed_time(b) for a, b in zip(e0, e1))
+
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(args.steps):
-        step()
-    e1.record(stream)
-    barrier()
-    ms = e0.elapsed_time(e1)
+    ms = timed(args.steps, fits_l2)
     clocks = sampler.stop() if rank == 0 else {}
     ms_step = max_over_ranks(ms, world, "cuda") / args.steps
-    value = aggregate_value(N * n, world, ms_step)
+    value = aggregate_value(voxel_iters, world, ms_step)
+    l2_note = {"working_set_mb": 2 * N * 4 / 1e6, "timed": "larger than L2: back to back, no flush needed"}
+    if fits_l2:
+        ms_warm = max_over_ranks(timed(args.steps, False), world, "cuda") / args.steps
+        l2_note = {"working_set_mb": 2 * N * 4 / 1e6, "timed": "cold: 512 MB scratch write between timed calls (value)",
+                   "warm_ms_per_step": ms_warm, "warm_value": aggregate_value(voxel_iters, world, ms_warm),
+                   "cold_ms_per_step": ms_step}
+    extra = {}
+    if sweep:                                 # the same exploration run incrementally: 40 single-iteration calls (pin P11)
+        cur = d_in.clone()
+
+        def inc():
+            cur.copy_(d_in)
+            for _ in range(n):
+                B.idg_filter_batched(cur, 1, plist, out=cur, workspace=ws, stream=stream)
+        for _ in range(2):
+            inc()
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.steps):
+            inc()
+        e1.record(stream)
+        barrier()
+        ms_inc = max_over_ranks(e0.elapsed_time(e1), world, "cuda") / args.steps
+        extra["incremental_sweep"] = {"ms_per_sweep": ms_inc, "value": aggregate_value(N * n, world, ms_inc), "unit": UNIT,
+                                      "what": f"{n} single-iteration batched calls in place (warm), {nb} cubes", "plan": B.idg_last_plan()}
 
     # end to end through the C-ABI host entry point: pinned host buffers, copies inside the timed region
-    e2e_value = None
+    e2e_value, e2e_floor = None, None
     if not args.no_e2e:
         host_out = torch.empty_like(host_in).pin_memory()
         dev = torch.empty(B.host_buffers_bytes(nx, ny, nz), dtype=torch.uint8, device="cuda")
@@ -308,6 +387,7 @@ def run_ours(args) -> None:
             B.idg_filter_host(host_in, n, p, out_host=host_out, dev_buffers=dev, stream=stream)
         barrier()
         e_steps = max(2, min(args.steps, 5))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         t0 = time.perf_counter()
         e0.record(stream)
         for _ in range(e_steps):
@@ -315,7 +395,30 @@ def run_ours(args) -> None:
         e1.record(stream)
         barrier()
         e_ms = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3)
-        e2e_value = aggregate_value(N * n, world, max_over_ranks(e_ms, world, "cuda") / e_steps)
+        e2e_value = aggregate_value(voxel_iters, world, max_over_ranks(e_ms, world, "cuda") / e_steps)
+        # its floor, measured: the same bytes over the same link with no kernel at all -- upload of the cube and
+        # download of a cube on two streams at once, in the slabs the pipeline uses
+        s_up, s_dn = torch.cuda.Stream(), torch.cuda.Stream()
+        slabs = 16 if N * 4 >= (64 << 20) else 1
+        zs = -(-nz // slabs)
+        d_tmp = d_out
+
+        def copies():
+            for z in range(0, nz, zs):
+                with torch.cuda.stream(s_up):
+                    d_in[z:z + zs].copy_(host_in[z:z + zs], non_blocking=True)
+                with torch.cuda.stream(s_dn):
+                    host_out[z:z + zs].copy_(d_tmp[z:z + zs], non_blocking=True)
+        copies()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e_steps):
+            copies()
+        barrier()
+        f_ms = max_over_ranks((time.perf_counter() - t0) * 1e3, world, "cuda") / e_steps
+        e2e_floor = {"ms_per_step": f_ms, "value": aggregate_value(voxel_iters, world, f_ms),
+                     "what": f"copy-only pipeline: H2D and D2H of {N * 4 / 1e9:.2f} GB each, {slabs} slabs, two streams, no kernel",
+                     "frac": f_ms / (max_over_ranks(e_ms, world, "cuda") / e_steps)}
 
     if rank != 0:
         if world > 1:
@@ -326,10 +429,12 @@ def run_ours(args) -> None:
     ms_launch = ms_step / launches_per_step
     if filt is not None and filt[0] == "wavelet":      # many small passes: the roofline unit is the whole filter
         ms_launch, fuse = ms_step, 1
-    achieved = BYTES_PER_VOXEL_ITER * N * fuse / (ms_launch * 1e-3) / 1e9     # algorithmic GB/s per launch
-    kernel_tag = f"{plan} {args.workload}"
+    alg_bytes = BYTES_PER_VOXEL_ITER * voxel_iters / launches_per_step        # algorithmic bytes per launch
+    hbm_equiv = alg_bytes / (ms_launch * 1e-3) / 1e9
+    ncu = ncu_counters(plan, args.workload)
+    traffic = ncu.get("dram_bytes")
+    import oracle
     if filt is not None:                      # reference filter: its own metric, oracle timed on a small block
-        import oracle
         cores = oracle.set_threads(os.cpu_count() or 1)
         blk = data[:min(nz, 48), :min(ny, 256), :min(nx, 256)]
         t0 = time.perf_counter()
@@ -348,42 +453,69 @@ def run_ours(args) -> None:
             oracle.gaussian_filter_oracle(blk, filt[1], filt[2])
         dt = time.perf_counter() - t0
         cpu_v, sample = blk.size / dt / 1e9, f"{blk.shape[2]}x{blk.shape[1]}x{blk.shape[0]} block, oracle as it stands, fp64, {dt:.1f} s"
+        cpu_1 = None
         metric, unit, params = f"{args.filter}_throughput", "Gvoxel/s", str(filt[1:])
     else:
-        first = data[0] if batched else data
-        cpu_v, cores, sample, _ = oracle_rate(first, n, 15.0, (plist[0] if batched else p).f32())
+        first = data[0] if nb > 1 else data
+        prm0 = (plist[0] if nb > 1 else p).f32()
+        n_cpu = 10 if sweep else n
+        cpu_v, cores, sample, _ = oracle_rate(first, n_cpu, 12.0, prm0)
+        v1, _, s1, _ = oracle_rate(first, n_cpu, 5.0, prm0, threads=1)
+        oracle.set_threads(os.cpu_count() or 1)
+        cpu_1 = {"value": v1, "unit": UNIT, "cores": 1, "sample": s1}
         metric, unit = METRIC, UNIT
         params = ("per-cube K, tau, C_j (synth.batch_params)" if batched
+                  else "K in {0.5,1,1.5,2,3,5,7.5,10} x S/N {22,62}, tau=0.0325 C=5, every n = 1..40 from scratch" if sweep
                   else "K=1.5 tau=0.0325 Cx=Cy=Cz=5 rms=1 (PAPER.md:187, :406)")
+
+    # Which ceiling binds.  The temporally fused IDG kernels are bound by FP32 issue, not by HBM:
+    # the roof is the SMs' instruction issue rate (148 SMs x 4 schedulers x 1.965 GHz, B200_PROFILING.md unit counts)
+    # and `achieved` is the MEASURED warp-instruction count of this plan (ncu, profiles/ncu_per_launch.json) over the
+    # launch time measured live here.  hbm_equiv_frac keeps north_star's figure (8 B per voxel-iteration over the
+    # copy bandwidth: > 1 means the fusion beats an un-fused sweep); dram_frac_actual is what really crosses the HBM pins.
+    issue_peak = 148 * 4 * 1.965e9 / 1e12              # T warp-instructions / s
+    fused_idg = filt is None and ("idg_tma" in plan or "idg_stream" in plan or "idg_resident" in plan) and fuse >= 2
+    roof = {"bound": "hbm", "achieved": hbm_equiv, "peak": peak, "unit": "GB/s", "frac": hbm_equiv / peak,
+            "traffic": traffic, "kernel": plan, "ms_per_launch": ms_launch,
+            "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src}
+    if fused_idg:
+        wi = ncu.get("warp_instructions")
+        roof.update({"bound": "alu", "unit": "T warp-inst/s", "peak": issue_peak,
+                     "achieved": (wi / (ms_launch * 1e-3) / 1e12) if wi else None,
+                     "frac": (wi / (ms_launch * 1e-3) / 1e12 / issue_peak) if wi else None,
+                     "peak_source": "derived: 148 SMs x 4 warp schedulers x 1.965 GHz (B200_PROFILING.md)",
+                     "warp_instructions_per_launch": wi,
+                     "useful_thread_inst_per_voxel_iter": (wi * 32 / (voxel_iters / launches_per_step)) if wi else None})
+    roof["hbm_equiv_gbs"] = hbm_equiv
+    roof["hbm_equiv_frac"] = hbm_equiv / peak
+    roof["hbm_peak_gbs"] = peak
+    roof["dram_frac_actual"] = (traffic / (ms_launch * 1e-3) / 1e9 / peak) if traffic else None
+    roof["counters_source"] = ({k: ncu[k] for k in ("source", "commit") if k in ncu} if ncu else
+                               "no ncu capture of this plan on this workload is committed: traffic and the ALU figures are withheld")
+    if fits_l2:
+        l2b = ncu.get("l2_bytes")
+        roof["l2"] = {"bytes_per_launch": l2b, "gbs": (l2b / (ms_launch * 1e-3) / 1e9) if l2b else None,
+                      "peak_gbs": L2_PEAK_GBS, "frac": (l2b / (ms_launch * 1e-3) / 1e9 / L2_PEAK_GBS) if l2b else None,
+                      "note": "lts__t_bytes.sum of the ncu capture over the launch time measured here"}
+    roof["note"] = ("algorithmic bytes = 8 B x voxel-iterations of a launch (what an un-fused sweep must move); temporal "
+                    "fusion moves fewer DRAM bytes, so hbm_equiv_frac can exceed 1 -- dram_frac_actual is the real HBM load")
     line = {
         "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps,
-        "warmup": max(3, args.warmup), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "warmup": warm, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": args.workload, "shape_xyz": [nx, ny, nz], "n_iter": n,
-                   "params": params, "batch": BATCH if batched else 1,
+                   "params": params, "batch": nb,
                    "fused_iterations_per_launch": fuse, "parallelism": f"replicas x{world}",
-                   "l2": f"input + output ({2 * N * 4 / 1e6:.0f} MB per call) against the 126 MB L2: "
-                         + ("larger, no flush needed" if 2 * N * 4 > 252e6 else "NOT larger -- warm-L2 number"),
-                   "paper_context": "GTX860M OpenGL 0.90, i7 8 threads 0.036 Gvoxel-iter/s (PAPER.md:408-414)"},
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": ncu_traffic_bytes(kernel_tag),
-                     "kernel": plan, "ms_per_launch": ms_launch,
-                     "algorithmic_bytes_per_launch": BYTES_PER_VOXEL_ITER * N * fuse,
-                     "peak_source": peak_src,
-                     "note": "algorithmic bytes = 8 B x voxels x fused iterations (what an un-fused sweep must "
-                             "move); temporal fusion moves fewer DRAM bytes, so frac can exceed 1 -- see traffic"},
-        "cpu_baseline": {"value": cpu_v, "unit": unit, "cores": cores, "kind": "oracle", "sample": sample},
+                   "l2": l2_note,
+                   "paper_context": "GTX860M OpenGL 0.90, i7 8 threads 0.036 Gvoxel-iter/s (PAPER.md:408-414)", **extra},
+        "roofline": roof,
+        "cpu_baseline": {"value": cpu_v, "unit": unit, "cores": cores, "kind": "oracle", "sample": sample,
+                         "single_thread": cpu_1, "cpu_model": cpu_model()},
         "e2e": {"value": e2e_value, "unit": unit, "h2d_bytes_per_step": N * 4, "d2h_bytes_per_step": N * 4,
-                "api": "idg_filter_host (pinned host buffers)"},
+                "api": "idg_filter_host (pinned host buffers)", "floor": e2e_floor},
         "gpu_launches": launches_per_step * args.steps,
         "clocks": clocks,
     }
-    if filt is None:
-        # after temporal fusion the IDG kernels sit between the DRAM and the FP32 ceilings: report the second too
-        lane_ops = 10.0 * value * 1e9 / 1e12                       # 10 FP32 lane-ops per voxel-iteration
-        peak_ops = 148 * 128 * 1.965e9 / 1e12
-        line["roofline"]["alu"] = {"achieved": lane_ops, "peak": peak_ops, "unit": "T lane-op/s", "frac": lane_ops / peak_ops,
-                                   "note": "useful voxel-iterations only; halo recomputation (x 1.2 at T = 2 to x 1.45 at T = 4) comes on top"}
     if filt is not None and filt[0] == "gauss" and any(filt[2]):     # rotated Gaussian: bound by FP32, not by HBM
         r = B.idg_gaussian_radii(filt[1], filt[2])[0]
         flops = 2.0 * (2 * r + 1) ** 3 * N
@@ -406,6 +538,7 @@ def main() -> None:
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--filter", default="idg", choices=sorted(FILTERS),
                     help="idg (the contract's metric) or a reference filter: one pass, Gvoxel/s")
+    ap.add_argument("--kernel", type=int, default=0, help="IDG_OPT_KERNEL (0 = library default plan)")
     ap.add_argument("--fuse", type=int, default=0, help="iterations fused per launch (0 = library default)")
     ap.add_argument("--zchunk", type=int, default=0, help="planes per CTA along z (0 = library default)")
     ap.add_argument("--tile", type=int, default=0, help="TMA kernel tile variant (0 = library default)")

@@ -38,7 +38,7 @@
 extern "C" {
 #endif
 
-#define IDG_VERSION 100            /* major*10000 + minor*100 + patch */
+#define IDG_VERSION 10100           /* major*10000 + minor*100 + patch */
 
 enum {
     IDG_OK = 0,
@@ -81,8 +81,11 @@ unsigned idg_params_check(const idg_params *params /*[host]*/);
 /*
  * Bytes of device workspace idg_filter_ws / idg_filter_batched need for `batch`
  * cubes of nx*ny*nz voxels: one scratch cube per cube (the "temporary eta" of
- * PAPER.md:430) plus a small parameter table and the 256-byte block holding the
- * arrival counter of the cooperative single-launch path.  0 on invalid dimensions.
+ * PAPER.md:430) plus a small parameter table, the 256-byte block holding the
+ * arrival counter of the cooperative single-launch path and, for cubes the resident
+ * kernel can take (nx % 4 == 0, at most 4 Mi voxels), 32 MB of mailboxes for the
+ * block faces.  0 on invalid dimensions.  A batch of more than ~2000 cubes uploads
+ * its parameter table from pageable memory, which may synchronise the host.
  */
 size_t idg_workspace_bytes(int nx, int ny, int nz, int batch);
 
@@ -135,7 +138,9 @@ int idg_filter_batched(const float *cubes, int nx, int ny, int nz, int batch,
  * I_n to out_host and synchronises `stream` before returning.  Cubes of 64 MB
  * and more are cut into up to 16 z slabs (each filtered with n_iter halo planes
  * per side, bit-identical results) so that upload, filtering and download
- * overlap on two internal copy streams; pinned host memory is needed for that.
+ * overlap on two copy streams created (and destroyed) by the call on the current
+ * device; pinned host memory is needed for that.  Safe to call from several host
+ * threads and on several devices at once: no state is shared between calls.
  *   cube_host, out_host [host] nx*ny*nz fp32 (pinned memory gives full PCIe rate)
  *   dev_buffers [device] 2*nx*ny*nz*4 + idg_workspace_bytes(nx,ny,nz,1) bytes,
  *               256-byte aligned, or NULL to use the stream-ordered allocator.
@@ -206,6 +211,12 @@ int idg_mask_sums(const float *orig, const float *filt, const float *model, int 
 int idg_cube_stats(const float *cube, int nx, int ny, int nz, const idg_roi *roi, double *stats, void *stream);
 
 /*
+ * Host-only: mean and noise level rms = sqrt(<x^2> - <x>^2) (reading Q4) from a HOST copy of the
+ * idg_cube_stats output.  Either output pointer may be NULL; n = 0 gives NaN.  IDG_ERR_NULL for stats == NULL.
+ */
+int idg_stats_rms(const double *stats, double *mean, double *rms);
+
+/*
  * Histogram of the voxel intensities of the ROI (Fig. 6): `nbins` (1..8192) equal bins over
  * [lo, hi); a voxel v with lo <= v < hi (and v >= *mask_thr when mask_thr is given) counts in bin
  * floor((v - lo) * (nbins / (hi - lo))), every operation in fp32 (reading Q5); NaN never counts.
@@ -258,19 +269,24 @@ int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, i
                        float rms, float *out, void *stream);
 
 /*
- * Process-wide tuning knobs (tests and benchmarks; defaults give the fastest plan).
- *   IDG_OPT_KERNEL   0 auto (kernel 3 wherever nx % 4 == 0 and the buffers are 16-byte aligned) | 1 naive (one
- *                    thread per voxel) | 2 tiled z-streaming kernel (global loads) | 3 tiled z-streaming kernel
- *                    fed by TMA (the fast path) | 4 persistent warp-decoupled TMA kernel.  Reference filters: 1 = the
+ * Tuning knobs of the CALLING HOST THREAD (tests and benchmarks; defaults give the fastest plan): an option set by
+ * one thread affects the calls that thread makes afterwards and no other thread's.
+ *   IDG_OPT_KERNEL   0 auto (the resident kernel 5 when the whole call fits in the SMs' shared memory at once, else
+ *                    kernel 3 wherever nx % 4 == 0 and the buffers are 16-byte aligned) | 1 naive (one thread per
+ *                    voxel) | 2 tiled z-streaming kernel (global loads) | 3 tiled z-streaming kernel fed by TMA (the
+ *                    fast path for large cubes) | 4 (retired: runs kernel 3) | 5 resident kernel: blocks of
+ *                    the cube(s) stay in shared memory for all iterations of the call, block faces are exchanged
+ *                    through mailboxes in the workspace, one cooperative launch per wave of cubes (cubes of up to
+ *                    4 Mi voxels with nx % 4 == 0, nx >= 8; otherwise the auto plan).  Reference filters: 1 = the
  *                    general separable kernel also where the TMA-fed one applies.  Wavelets: see idg_wavelet_filter
  *   IDG_OPT_FUSE     0 auto (4, or 2 for full-GPU workloads of cubes thinner than 100 planes) | 1..4 = diffusion
  *                    iterations fused per launch (kernels 2-4)
  *   IDG_OPT_ZCHUNK   0 auto | >0  = planes per CTA along z (kernels 2, 3)
  *   IDG_OPT_TILE     0 auto | kernel 3: 1 = one CTA per SM (T <= 2: 128x64 tile, 512 threads; T >= 3: 128x32
  *                    tile, 256 threads), 2 = 128x32 tile, two 256-thread CTAs per SM (T <= 2), 3 = 384-thread CTA
- *                    (T >= 3) | kernel 4: 1..4, see idg_stream.cu | separable reference filters: 2 = strips of 4
+ *                    (T >= 3) | separable reference filters: 2 = strips of 4
  *                    rows per thread instead of 2 in idg_sep3d_tma_kernel
- *   IDG_OPT_CTAS     0 auto | >0  = persistent grid size of kernel 4
+ *   IDG_OPT_CTAS     reserved (was the grid size of the retired kernel 4); ignored
  *   IDG_OPT_HOST_SLABS  0 auto | 1..16 = z slabs of the idg_filter_host transfer/compute pipeline (1 = one piece)
  *   IDG_OPT_COOP     0 auto (small cubes whose whole grid is co-resident: all launches of kernel 3 folded into ONE
  *                    cooperative launch with grid barriers between the fused rounds) | 1 never | 2 whenever the grid fits
@@ -284,9 +300,12 @@ int idg_get_option(int key);
 /*
  * Stream-ordered temporaries (the scratch cube of idg_filter, the device buffers of idg_filter_host when none
  * are passed, the kernel weights of a rotated Gaussian, the lattices of the Le Gall filter) come from a memory
- * pool private to the library, one per device, which keeps the memory it has been given between calls so that
- * a call does not pay the driver's map / unmap again.  idg_release_temporaries() returns everything that is not
- * in use on the current device to the driver (synchronise the streams that used the library first).
+ * pool private to the library, one per device, which keeps memory between calls so that a call does not pay the
+ * driver's map / unmap again -- at most twice the size of the largest recent request, halved after every 64
+ * requests in a row below a quarter of it (so a 2 GB temporary is not held for ever once the caller moves on to
+ * small cubes).
+ * idg_release_temporaries() returns everything that is not in use on the current device to the driver at once
+ * (synchronise the streams that used the library first).
  * Returns IDG_OK or a cudaError_t.
  */
 int idg_release_temporaries(void);

@@ -26,7 +26,7 @@ SYMBOLS = ("idg_version", "idg_status_string", "idg_params_check", "idg_workspac
            "idg_set_option", "idg_get_option", "idg_last_launch_count", "idg_last_plan",
            "idg_box_filter", "idg_gaussian_filter", "idg_gaussian_radii",
            "idg_mask_sums", "idg_cube_stats", "idg_quality", "idg_filter_pm",
-           "idg_wavelet_transform", "idg_wavelet_filter", "idg_histogram", "idg_release_temporaries")
+           "idg_wavelet_transform", "idg_wavelet_filter", "idg_histogram", "idg_release_temporaries", "idg_stats_rms")
 WAVELET_HAAR, WAVELET_LEGALL53 = 0, 1
 
 
@@ -117,6 +117,8 @@ def lib() -> ctypes.CDLL:
         L.idg_cube_stats.argtypes = [fp, i, i, i, rp, vp, vp]
         L.idg_histogram.restype = i
         L.idg_histogram.argtypes = [fp, i, i, i, rp, f, f, i, ctypes.POINTER(ctypes.c_float), vp, vp]
+        L.idg_stats_rms.restype = i
+        L.idg_stats_rms.argtypes = [dptr, dptr, dptr]
         L.idg_quality.restype = i
         L.idg_quality.argtypes = [dptr, d, d, d, dptr, dptr, dptr]
         L.idg_wavelet_transform.restype = i
@@ -341,6 +343,14 @@ def idg_cube_stats(cube: torch.Tensor, roi=None, stats: Optional[torch.Tensor] =
     _check(lib().idg_cube_stats(_dev(cube, "cube"), nx, ny, nz, None if r is None else ctypes.byref(r),
                                 stats.data_ptr(), _stream(stream)))
     return stats
+
+
+def idg_stats_rms(stats: Sequence[float]) -> tuple:
+    """idg_stats_rms on a HOST copy of the idg_cube_stats output: (mean, rms)."""
+    arr = (ctypes.c_double * 8)(*[float(v) for v in list(stats)[:8]] + [0.0] * (8 - min(8, len(stats))))
+    mean, rms = ctypes.c_double(), ctypes.c_double()
+    _check(lib().idg_stats_rms(arr, ctypes.byref(mean), ctypes.byref(rms)))
+    return mean.value, rms.value
 
 
 def idg_histogram(cube: torch.Tensor, lo: float, hi: float, nbins: int, roi=None, mask_thr: Optional[float] = None,

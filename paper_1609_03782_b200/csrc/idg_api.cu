@@ -12,7 +12,7 @@
 
 namespace {
 
-int g_opt[IDG_OPT_COUNT_] = {0, 0, 0, 0, 0, 0, 0};
+thread_local int g_opt[IDG_OPT_COUNT_] = {0, 0, 0, 0, 0, 0, 0};      // tuning knobs of the calling host thread
 thread_local int t_launches = 0;
 thread_local char t_plan[96] = "none";
 
@@ -98,7 +98,6 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     // Plan: kernel variant and iterations fused per launch.
     const bool can_tile = idg::tiled_supported(nx, ny, nz, cubes, out, scratch);
     const bool can_tma = idg::tma_supported(nx, ny, nz, cubes, out, scratch);
-    const bool can_stream = idg::stream_supported(nx, ny, nz, cubes, out, scratch);
     int kernel = g_opt[IDG_OPT_KERNEL];
     int fuse = g_opt[IDG_OPT_FUSE];
     int tile = g_opt[IDG_OPT_TILE];
@@ -129,22 +128,17 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
             kernel = can_tile ? 2 : 1;
         }
     }
-    if (mode == 1 && kernel != 5) {          // gradient-driven variant: kernel 3 (any T), the persistent kernel (option 4, T <= 2) or the naive kernel
+    if (mode == 1 && kernel != 5) {          // gradient-driven variant: kernel 3 (any T) or the naive kernel
         const int ko = g_opt[IDG_OPT_KERNEL];
         fuse = g_opt[IDG_OPT_FUSE];
-        if ((ko == 0 || ko == 3) && can_tma) {
+        if ((ko == 0 || ko == 3 || ko == 4) && can_tma) {
             kernel = 3;
             if (!fuse) fuse = (nz < 100 && (double)N * (double)batch >= 4.0e6) ? 2 : 4;
-        } else if (ko != 1 && can_stream) {
-            kernel = 4;
-            if (fuse > 2 || fuse == 0) fuse = 2;
-            tile = g_opt[IDG_OPT_TILE];
-            if (tile > 2 || tile == 0) tile = ((double)N * (double)batch < 6.4e7) ? 2 : 1;
         } else {
             kernel = 1;
         }
     }
-    if (kernel == 4 && !can_stream) kernel = 2;
+    if (kernel == 4) kernel = can_tma ? 3 : 2;      // kernel 4 (persistent warp-decoupled variant) was retired in 1.1
     if (kernel == 3 && !can_tma) kernel = 2;
     if (kernel == 2 && !can_tile) kernel = 1;
     if (kernel == 5) {
@@ -157,7 +151,7 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     }
     {
         static const char *const names[6] = {"", "idg_naive_kernel", "idg_tiled_kernel", "idg_tma_kernel",
-                                             "idg_stream_kernel", "idg_resident_kernel"};
+                                             "", "idg_resident_kernel"};
         snprintf(t_plan, sizeof(t_plan), "%s%s fuse=%d tile=%d", names[kernel], mode == 1 ? " pm" : "", fuse, tile);
     }
 
@@ -248,8 +242,7 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
             if (tile_now == 0) tile_now = L.fuse <= 2 ? 2 : (L.fuse == 3 ? 3 : 1);
             else if (L.fuse <= 2 && tile_now > 2) tile_now = 0;
         }
-        e = (kernel == 4)   ? idg::launch_stream(L, g_opt[IDG_OPT_CTAS], tile, st)
-            : (kernel == 3) ? idg::launch_tma(L, g_opt[IDG_OPT_ZCHUNK], tile_now, st)
+        e = (kernel == 3)   ? idg::launch_tma(L, g_opt[IDG_OPT_ZCHUNK], tile_now, st)
             : (kernel == 2) ? idg::launch_tiled(L, g_opt[IDG_OPT_ZCHUNK], st)
                             : idg::launch_naive(L, st);
         if (e != cudaSuccess) return (int)e;
@@ -341,6 +334,36 @@ int idg_filter(const float *cube, int nx, int ny, int nz, int n_iter, const idg_
 
 constexpr int kMaxSlabs = 16;      // z slabs of the idg_filter_host pipeline
 
+// Streams and events of one idg_filter_host call (destroyed when the call returns; the destructor runs after the
+// call has synchronised both copy streams).
+struct SlabSync {
+    cudaStream_t h2d = nullptr, d2h = nullptr;
+    cudaEvent_t ev_h[kMaxSlabs] = {}, ev_c[kMaxSlabs] = {}, ev_d[kMaxSlabs] = {}, begin = nullptr;
+    cudaError_t create(int slabs)
+    {
+        cudaError_t e = cudaStreamCreateWithFlags(&h2d, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&d2h, cudaStreamNonBlocking);
+        for (int i = 0; i < slabs && i < kMaxSlabs && e == cudaSuccess; ++i) {
+            e = cudaEventCreateWithFlags(&ev_h[i], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_c[i], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_d[i], cudaEventDisableTiming);
+        }
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&begin, cudaEventDisableTiming);
+        return e;
+    }
+    ~SlabSync()
+    {
+        for (int i = 0; i < kMaxSlabs; ++i) {
+            if (ev_h[i]) cudaEventDestroy(ev_h[i]);
+            if (ev_c[i]) cudaEventDestroy(ev_c[i]);
+            if (ev_d[i]) cudaEventDestroy(ev_d[i]);
+        }
+        if (begin) cudaEventDestroy(begin);
+        if (h2d) cudaStreamDestroy(h2d);
+        if (d2h) cudaStreamDestroy(d2h);
+    }
+};
+
 int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
                     const idg_params *params, float *out_host, void *dev_buffers,
                     size_t dev_buffers_bytes, void *stream)
@@ -394,20 +417,12 @@ int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
     const size_t slab_al = align_up((size_t)max_planes * plane_b);
     const size_t slab_ws = idg_workspace_bytes(nx, ny, max_planes, 1);
     if (slabs > 1 && n_iter > 0 && 2 * slab_al + slab_ws <= need - cube_al) {
-        static cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
-        static cudaEvent_t ev_h[kMaxSlabs], ev_c[kMaxSlabs], ev_d[kMaxSlabs], ev_begin;
-        static bool ready = false;
-        if (!ready) {
-            e = cudaStreamCreateWithFlags(&s_h2d, cudaStreamNonBlocking);
-            if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s_d2h, cudaStreamNonBlocking);
-            for (int i = 0; i < kMaxSlabs && e == cudaSuccess; ++i) {
-                e = cudaEventCreateWithFlags(&ev_h[i], cudaEventDisableTiming);
-                if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_c[i], cudaEventDisableTiming);
-                if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_d[i], cudaEventDisableTiming);
-            }
-            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_begin, cudaEventDisableTiming);
-            ready = (e == cudaSuccess);
-        }
+        // two copy streams and the per-slab events of THIS call on the CURRENT device (nothing shared between
+        // callers, host threads or devices); created per call: a call that gets here moves >= 64 MB each way
+        SlabSync sync;
+        e = sync.create(slabs);
+        cudaStream_t s_h2d = sync.h2d, s_d2h = sync.d2h;
+        cudaEvent_t *ev_h = sync.ev_h, *ev_c = sync.ev_c, *ev_d = sync.ev_d, ev_begin = sync.begin;
         char *region = base + cube_al;
         float *d_slab[2] = {(float *)region, (float *)(region + slab_al)};
         void *ws_slab = region + 2 * slab_al;
@@ -653,6 +668,15 @@ int idg_cube_stats(const float *cube, int nx, int ny, int nz, const idg_roi *roi
     if (e != cudaSuccess) return (int)e;
     t_launches = 1;
     snprintf(t_plan, sizeof(t_plan), "idg_cube_stats_kernel");
+    return IDG_OK;
+}
+
+int idg_stats_rms(const double *stats, double *mean, double *rms)
+{
+    if (!stats) return IDG_ERR_NULL;
+    const double n = stats[0], m = n > 0.0 ? stats[1] / n : NAN;
+    if (mean) *mean = m;
+    if (rms) *rms = n > 0.0 ? sqrt(fmax(stats[2] / n - m * m, 0.0)) : NAN;
     return IDG_OK;
 }
 

@@ -81,11 +81,10 @@ cudaError_t launch_r(const ConvArgs &S, cudaStream_t st)
     constexpr int W = 2 * R + 1, BZ = bz_of(R);
     constexpr size_t smem = sizeof(float) * ((size_t)(BX + 2 * R) * (BY + 2 * R) * (BZ + 2 * R) + (size_t)W * W * W);
     static_assert(smem <= 227u * 1024u, "shared memory budget");
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(idg_conv3d_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static DeviceOnce smem_once;
+    {
+        const cudaError_t e = set_max_dynamic_smem(smem_once, (const void *)(idg_conv3d_kernel<R>), smem);
         if (e != cudaSuccess) return e;
-        attr_done = true;
     }
     const unsigned gx = (unsigned)((S.nx + BX - 1) / BX), gy = (unsigned)((S.ny + BY - 1) / BY),
                    gz = (unsigned)((S.nz + BZ - 1) / BZ);

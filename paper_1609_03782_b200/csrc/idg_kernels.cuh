@@ -110,8 +110,6 @@ cudaError_t launch_tma(const Launch &L, int zchunk, int tile, cudaStream_t st);
 // cudaErrorNotSupported / cudaErrorCooperativeLaunchTooLarge: use launch_tma per round instead.
 cudaError_t launch_tma_coop(const Launch &L, int zchunk, int tile, int rounds, unsigned *bar, cudaStream_t st);
 bool tma_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
-cudaError_t launch_stream(const Launch &L, int nctas, int tile, cudaStream_t st);
-bool stream_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
 
 // Resident kernel (idg_resident.cu): the cube(s) stay in shared memory for all iterations of a call; block faces are
 // exchanged through mailboxes in the workspace.  resident_plan() picks the block decomposition (false: the shape does
@@ -130,6 +128,13 @@ bool resident_plan(int nx, int ny, int nz, int batch, int max_n, size_t mail_byt
 cudaError_t launch_resident(const Launch &L, const ResidentPlan &P, unsigned long long *mail, cudaStream_t st,
                             int *launches);
 int device_sm_count();      // SMs of the current device (148 when it cannot be queried)
+
+// Per-device one-time work (idg_tmap.cu).  cudaFuncSetAttribute applies to the CURRENT device only, so "done" is
+// remembered per device ordinal; a benign race just sets the attribute twice.
+struct DeviceOnce {
+    unsigned long long done_mask[4] = {0, 0, 0, 0};      // devices 0..255
+};
+cudaError_t set_max_dynamic_smem(DeviceOnce &once, const void *kernel, size_t bytes);
 
 // Stream-ordered temporaries (idg_tmap.cu): cudaMallocAsync from a private memory pool that keeps what it has
 // been given (release threshold = everything), so a call that needs a cube-sized temporary does not pay the

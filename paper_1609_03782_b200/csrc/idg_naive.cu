@@ -37,7 +37,7 @@ cudaError_t launch_naive(const Launch &L, cudaStream_t st)
 {
     const size_t N = (size_t)L.nx * L.ny * L.nz;
     size_t blocks = (N + 255) / 256;
-    if (blocks > 148u * 64u) blocks = 148u * 64u;      // grid-stride beyond 64 CTAs per SM
+    if (blocks > (unsigned)device_sm_count() * 64u) blocks = (unsigned)device_sm_count() * 64u;      // grid-stride beyond 64 CTAs per SM
     dim3 grid((unsigned)blocks, (unsigned)L.batch);
     idg_naive_kernel<<<grid, 256, 0, st>>>(L);
     return cudaGetLastError();

@@ -88,19 +88,13 @@ __device__ __forceinline__ uint32_t atom_add_acq_rel(uint32_t addr, uint32_t v)
     asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(addr), "r"(v) : "memory");
     return old;
 }
-// relaxed counter: enough for handing back a buffer that was only READ (the loaded values have
-// been consumed by the time the counter is bumped), as with a consumer-release mbarrier arrive
-__device__ __forceinline__ uint32_t atom_add_relaxed(uint32_t addr, uint32_t v)
-{
-    uint32_t old;
-    asm volatile("atom.relaxed.cta.shared::cta.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(addr), "r"(v) : "memory");
-    return old;
-}
 // Grid-wide barrier for cooperative launches (all CTAs co-resident): `bar` counts arrivals monotonically, `target`
 // = CTAs x barriers passed so far.  Global data written before it by any CTA (generic proxy) may afterwards be read
 // by any CTA, also through TMA (async proxy).
 __device__ __forceinline__ void grid_barrier(unsigned *bar, unsigned target)
 {
+    __threadfence();                                          // every thread: its global stores, for the generic ...
+    asm volatile("fence.proxy.async.global;" ::: "memory");   // ... and the async proxy (the next round reads by TMA)
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();

@@ -154,7 +154,7 @@ __global__ void __launch_bounds__(NT) idg_histogram_kernel(const __grid_constant
 unsigned grid_for(long long rows)
 {
     long long g = (rows + WARPS - 1) / WARPS;
-    const long long cap = 148LL * 8;                         // 8 CTAs of 256 threads per SM
+    const long long cap = (long long)device_sm_count() * 8;                         // 8 CTAs of 256 threads per SM
     if (g > cap) g = cap;
     return (unsigned)(g < 1 ? 1 : g);
 }

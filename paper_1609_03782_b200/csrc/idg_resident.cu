@@ -367,19 +367,6 @@ DevInfo dev_info()
 
 }  // namespace
 
-int device_sm_count()
-{
-    thread_local int cached_dev = -1, cached_sms = 148;
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return 148;
-    if (dev != cached_dev) {
-        const DevInfo d = dev_info();
-        cached_sms = d.sms > 0 ? d.sms : 148;
-        cached_dev = dev;
-    }
-    return cached_sms;
-}
-
 // Cost model (SM cycles per wave, calibrated on B200: profiles/r2a_notes.md): a cell costs ~18 clk of shared-memory
 // bandwidth per warp, a face entry ~24, an iteration ~700 of exchange latency and barrier; load + store + launch.
 namespace {

@@ -197,12 +197,10 @@ template <int RXY, int RZ>
 cudaError_t launch_class(const SepArgs &S, dim3 grid, cudaStream_t st)
 {
     using G = Geo<RXY, RZ>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(idg_sep3d_kernel<RXY, RZ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)G::kSmem);
+    static DeviceOnce smem_once;
+    {
+        const cudaError_t e = set_max_dynamic_smem(smem_once, (const void *)(idg_sep3d_kernel<RXY, RZ>), G::kSmem);
         if (e != cudaSuccess) return e;
-        attr_done = true;
     }
     idg_sep3d_kernel<RXY, RZ><<<grid, NT, G::kSmem, st>>>(S);
     return cudaGetLastError();
@@ -238,7 +236,7 @@ cudaError_t launch_sep3d(const float *in, float *out, int nx, int ny, int nz, in
     for (int i = 0; i <= 2 * rz; ++i) S.wz[i + cz - rz] = wz[i];
     const int tiles_x = (nx + TX - 1) / TX, tiles_y = (ny + TY - 1) / TY;
     // z chunks: minimise waves x (planes per chunk + warm-up planes) for ~3 resident CTAs per SM
-    const long tiles = (long)tiles_x * tiles_y, slots = 148L * 3;
+    const long tiles = (long)tiles_x * tiles_y, slots = (long)device_sm_count() * 3;
     long best_cost = -1;
     int chunks = 1;
     for (int c = 1; c <= nz && c <= 4096; ++c) {

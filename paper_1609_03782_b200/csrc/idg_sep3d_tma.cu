@@ -232,16 +232,15 @@ cudaError_t launch_cfg(SepTmaArgs &S, const float *in, int zchunk, cudaStream_t 
     const long tiles_y = (S.ny + G::VY - 1) / G::VY;
     const long tiles = (long)S.tiles_x * tiles_y;
     if (tiles > 0x7fffffffL) return cudaErrorInvalidValue;
-    S.zchunk = zchunk > 0 ? (zchunk < S.nz ? zchunk : S.nz) : pick_zchunk(S.nz, tiles, RZ, 148L * MINB);
+    S.zchunk = zchunk > 0 ? (zchunk < S.nz ? zchunk : S.nz) : pick_zchunk(S.nz, tiles, RZ, (long)device_sm_count() * MINB);
     if ((S.nz + S.zchunk - 1) / S.zchunk > 65535) S.zchunk = (S.nz + 65534) / 65535;
     CUtensorMap map;
     if (!tmap_encode(&map, in, S.nx, S.ny, S.nz, 1, kTileX, G::ROWS)) return cudaErrorNotSupported;
     auto kern = idg_sep3d_tma_kernel<RXY, RZ, R, WARPS, NS, MINB>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::kBytes);
+    static DeviceOnce smem_once;
+    {
+        const cudaError_t e = set_max_dynamic_smem(smem_once, (const void *)(kern), G::kBytes);
         if (e != cudaSuccess) return e;
-        attr_done = true;
     }
     const dim3 grid((unsigned)tiles, (unsigned)((S.nz + S.zchunk - 1) / S.zchunk));
     kern<<<grid, WARPS * 32, G::kBytes, st>>>(S, map);

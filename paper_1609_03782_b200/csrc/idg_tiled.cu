@@ -196,16 +196,17 @@ idg_tiled_kernel(const __grid_constant__ Launch L, const __grid_constant__ TileA
     else if (T > 3 && now == 3) tile_body<(T > 3 ? 3 : 1), R, WARPS>(src, dst, L, A, prm, edge);
 }
 
-// z-chunk length minimising waves * (planes per CTA) on 148 SMs with one CTA per SM.
+// z-chunk length minimising waves * (planes per CTA) with one CTA per SM of the current device.
 int pick_zchunk(int nz, int tiles, int T)
 {
+    const long sms = device_sm_count();
     long best_cost = -1;
     int best = nz;
     for (int nchunks = 1; nchunks <= nz; ++nchunks) {
         const int zc = (nz + nchunks - 1) / nchunks;
         const int real_chunks = (nz + zc - 1) / zc;
         const long ctas = (long)tiles * real_chunks;
-        const long waves = (ctas + 147) / 148;
+        const long waves = (ctas + sms - 1) / sms;
         const long cost = waves * (zc + 2 * T + 2);      // +2: per-CTA prologue, in plane-steps
         if (best_cost < 0 || cost < best_cost) {
             best_cost = cost;
@@ -232,11 +233,10 @@ cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st)
     if (chunks > 65535) A.zchunk = (L.nz + 65534) / 65535;
     const size_t smem = (size_t)T * 2 * WARPS * 2 * kLanes * sizeof(float4);
     auto kern = idg_tiled_kernel<T, R, WARPS>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static DeviceOnce smem_once;
+    {
+        const cudaError_t e = set_max_dynamic_smem(smem_once, (const void *)(kern), smem);
         if (e != cudaSuccess) return e;
-        attr_done = true;
     }
     dim3 grid((unsigned)tiles, (unsigned)((L.nz + A.zchunk - 1) / A.zchunk), (unsigned)L.batch);
     kern<<<grid, WARPS * 32, smem, st>>>(L, A);

@@ -178,6 +178,7 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
                     if (rev) nw[0][r] = F4{nw[0][r].w, nw[0][r].z, nw[0][r].y, nw[0][r].x};
                     sts4(const_cast<float *>(st) + cell[r], nw[0][r]);
                 }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // the stage is refilled by TMA later on
         }
         F4 out[R];
 #pragma unroll
@@ -315,17 +316,6 @@ int pick_zchunk(int nz, long tiles, int T, int slots, long max_ctas = 0)
     return best;
 }
 
-int sm_count()
-{
-    static int n = 0;
-    if (!n) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-            n = 0;
-    }
-    return n;
-}
-
 // rounds > 1: cooperative launch of all rounds (COOP instantiation); the grid must be co-resident.
 template <int T, int R, int WARPS, int NS, int MINB, bool COOP = false, bool PM = false>
 cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st, int rounds = 1, unsigned *bar = nullptr)
@@ -347,25 +337,23 @@ cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st, int rounds 
     void (*kern)(Launch, TmaArgs, Maps);
     if constexpr (COOP) kern = one ? idg_tma_coop_kernel<T, R, WARPS, NS, MINB, true> : idg_tma_coop_kernel<T, R, WARPS, NS, MINB, false>;
     else kern = one ? idg_tma_kernel<T, R, WARPS, NS, MINB, true, PM> : idg_tma_kernel<T, R, WARPS, NS, MINB, false, PM>;
-    static bool attr_done[2] = {false, false};
-    if (!attr_done[one]) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::kBytes);
+    static DeviceOnce smem_once[2];
+    {
+        const cudaError_t e = set_max_dynamic_smem(smem_once[one], (const void *)kern, S::kBytes);
         if (e != cudaSuccess) return e;
-        attr_done[one] = true;
     }
-    long slots = 148L * MINB;
+    const int sms = device_sm_count();
+    long slots = (long)sms * MINB;
     if (coop) {
-        static int per_sm[2] = {-1, -1};
-        if (per_sm[one] < 0 &&
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[one], kern, WARPS * 32, S::kBytes) != cudaSuccess)
-            per_sm[one] = 0;
-        slots = (long)per_sm[one] * sm_count();
+        int per_sm = 0;                      // of the current device (the cooperative path is rare: asked every time)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, WARPS * 32, S::kBytes) != cudaSuccess) per_sm = 0;
+        slots = (long)per_sm * sms;
         if (slots <= 0 || tiles * L.batch > slots) return cudaErrorCooperativeLaunchTooLarge;
         A.zchunk = pick_zchunk(L.nz, tiles * L.batch, T, (int)slots, slots);
         if (zchunk > 0 && tiles * L.batch * ((L.nz + zchunk - 1) / zchunk) <= slots) A.zchunk = zchunk < L.nz ? zchunk : L.nz;
         if (A.zchunk <= 0) return cudaErrorCooperativeLaunchTooLarge;
     } else {
-        A.zchunk = zchunk > 0 ? (zchunk < L.nz ? zchunk : L.nz) : pick_zchunk(L.nz, tiles * L.batch, T, 148 * MINB);
+        A.zchunk = zchunk > 0 ? (zchunk < L.nz ? zchunk : L.nz) : pick_zchunk(L.nz, tiles * L.batch, T, sms * MINB);
     }
     if ((L.nz + A.zchunk - 1) / A.zchunk > 65535) A.zchunk = (L.nz + 65534) / 65535;
     Maps M;

@@ -40,8 +40,6 @@ cudaMemPool_t temp_pool()
         props.location.id = dev;
         cudaMemPool_t p = nullptr;
         if (cudaMemPoolCreate(&p, &props) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
-        unsigned long long keep = ~0ull;
-        (void)cudaMemPoolSetAttribute(p, cudaMemPoolAttrReleaseThreshold, &keep);
         pool[dev] = p;
     }
     return pool[dev];
@@ -49,10 +47,60 @@ cudaMemPool_t temp_pool()
 
 }  // namespace
 
+cudaError_t set_max_dynamic_smem(DeviceOnce &once, const void *kernel, size_t bytes)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const bool tracked = dev >= 0 && dev < 256;
+    unsigned long long *word = &once.done_mask[tracked ? dev >> 6 : 0];
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (tracked && (__atomic_load_n(word, __ATOMIC_ACQUIRE) & bit)) return cudaSuccess;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess && tracked) __atomic_fetch_or(word, bit, __ATOMIC_RELEASE);
+    return e;
+}
+
+int device_sm_count()
+{
+    thread_local int cached_dev = -1, cached_sms = 148;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+    if (dev != cached_dev) {
+        int n = 0;
+        cached_sms = (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0) ? n : 148;
+        cached_dev = dev;
+    }
+    return cached_sms;
+}
+
+// What the pool may keep between calls (its release threshold) follows the requests: at least twice the largest
+// recent one; after 64 requests in a row that are all below a quarter of it, it is halved.  Repeated calls of one
+// size keep their temporaries mapped (no driver map / unmap per call); once the caller has moved on to small cubes
+// the memory of a large call goes back to the driver, so a co-resident allocator is not starved for ever.
 cudaError_t temp_alloc(void **p, size_t bytes, cudaStream_t st)
 {
     cudaMemPool_t pool = temp_pool();
-    return pool ? cudaMallocFromPoolAsync(p, bytes, pool, st) : cudaMallocAsync(p, bytes, st);
+    if (!pool) return cudaMallocAsync(p, bytes, st);
+    static unsigned long long keep[64] = {};
+    static int small_run[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64) {
+        unsigned long long thr = keep[dev];
+        if (2ull * bytes >= thr) {
+            thr = 2ull * bytes;
+            small_run[dev] = 0;
+        } else if (8ull * bytes < thr && ++small_run[dev] >= 64) {
+            thr /= 2;
+            small_run[dev] = 0;
+        }
+        if (thr != keep[dev]) {
+            keep[dev] = thr;
+            unsigned long long v = thr;
+            (void)cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &v);
+        }
+    }
+    return cudaMallocFromPoolAsync(p, bytes, pool, st);
 }
 
 cudaError_t temp_trim()

@@ -480,7 +480,7 @@ cudaError_t launch_phase(const WArgs &W, cudaStream_t st)
     const long long total = (long long)(W.axis == 0 ? nt : W.mx) * (W.axis == 1 ? nt : W.my) * (W.axis == 2 ? nt : W.mz);
     if (total <= 0 || m < 2) return cudaSuccess;
     long long grid = (total + NT - 1) / NT;
-    if (grid > 148LL * 32) grid = 148LL * 32;
+    if (grid > (long long)device_sm_count() * 32) grid = (long long)device_sm_count() * 32;
     idg_lift_kernel<WAVELET, PHASE, INV><<<(unsigned)grid, NT, 0, st>>>(W);
     return cudaGetLastError();
 }
@@ -502,7 +502,7 @@ cudaError_t transform(float *a, int nx, int ny, int nz, int levels, bool inverse
                 const long long total = (long long)(W.axis == 0 ? m / 2 : W.mx) * (W.axis == 1 ? m / 2 : W.my) *
                                         (W.axis == 2 ? m / 2 : W.mz);
                 long long grid = (total + NT - 1) / NT;
-                if (grid > 148LL * 32) grid = 148LL * 32;
+                if (grid > (long long)device_sm_count() * 32) grid = (long long)device_sm_count() * 32;
                 if (inverse) idg_haar_pair_kernel<true><<<(unsigned)grid, NT, 0, st>>>(W);
                 else idg_haar_pair_kernel<false><<<(unsigned)grid, NT, 0, st>>>(W);
                 e = cudaGetLastError();
@@ -516,13 +516,13 @@ cudaError_t transform(float *a, int nx, int ny, int nz, int levels, bool inverse
                     auto k = inverse ? idg_lift_xline_kernel<WAVELET, true> : idg_lift_xline_kernel<WAVELET, false>;
                     e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
                     long long grid = ((long long)W.my * W.mz + LW - 1) / LW;
-                    if (grid > 148LL * 16) grid = 148LL * 16;
+                    if (grid > (long long)device_sm_count() * 16) grid = (long long)device_sm_count() * 16;
                     if (e == cudaSuccess) k<<<(unsigned)grid, LW * 32, line_smem, st>>>(W);
                 } else {
                     auto k = inverse ? idg_lift_strip_kernel<WAVELET, true> : idg_lift_strip_kernel<WAVELET, false>;
                     e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
                     long long grid = (long long)((W.mx + SW - 1) / SW) * (W.axis == 1 ? W.mz : W.my);
-                    if (grid > 148LL * 16) grid = 148LL * 16;
+                    if (grid > (long long)device_sm_count() * 16) grid = (long long)device_sm_count() * 16;
                     if (e == cudaSuccess) k<<<(unsigned)grid, NT, line_smem, st>>>(W);
                 }
                 if (e == cudaSuccess) e = cudaGetLastError();
@@ -577,7 +577,7 @@ cudaError_t launch_wavelet_threshold(float *a, int nx, int ny, int nz, int level
     for (int i = 0; i < 16; ++i) T.thr[i] = i < levels ? thr[i] : 0.f;
     const size_t N = (size_t)nx * ny * (size_t)nz;
     size_t grid = (N + NT - 1) / NT;
-    if (grid > 148u * 32u) grid = 148u * 32u;
+    if (grid > (unsigned)device_sm_count() * 32u) grid = (unsigned)device_sm_count() * 32u;
     idg_wavelet_threshold_kernel<<<(unsigned)grid, NT, 0, st>>>(T);
     return cudaGetLastError();
 }

@@ -47,7 +47,7 @@ def explore(snr: float = 22.0, seed: int = 1001, nmax: int = 40, variant: str = 
             if n not in report:
                 continue
             st = B.idg_cube_stats(cur, noise_roi, stats).cpu().numpy()
-            rms_f = math.sqrt(max(st[2] / st[0] - (st[1] / st[0]) ** 2, 0.0))
+            rms_f = B.idg_stats_rms(st)[1]
             s = B.idg_mask_sums(orig, cur, model, 3.0 * c.rms, 3.0 * rms_f, roi, sums).cpu().numpy()
             q = B.idg_quality(s, c.rms, rms_f)
             rows.append({"K": float(K), "n": n, "rms_f": rms_f, **q})

@@ -32,7 +32,7 @@ def test_header_symbols_are_exported(binding):
 
 
 def test_version_and_status_strings(binding):
-    assert binding.idg_version() == 100
+    assert binding.idg_version() == 10100
     assert binding.status_string(0) == "ok"
     for s in range(-7, 0):
         assert binding.status_string(s) not in ("", "unknown status")
@@ -67,6 +67,47 @@ def test_options(binding):
         binding.idg_set_option(binding.IDG_OPT_FUSE, 9)
     with pytest.raises(IdgError):
         binding.idg_set_option(99, 0)
+
+
+def test_options_are_per_host_thread(binding):
+    """idg.h: an option set by one host thread affects that thread's calls only (thread_local state): two threads
+    holding different IDG_OPT_FUSE at the same time each read back their own, and the main thread's stays untouched."""
+    import threading
+    binding.idg_set_option(binding.IDG_OPT_FUSE, 1)
+    seen, gate = {}, threading.Barrier(2)
+
+    def worker(value):
+        assert binding.idg_get_option(binding.IDG_OPT_FUSE) == 0          # a new thread starts from the defaults
+        binding.idg_set_option(binding.IDG_OPT_FUSE, value)
+        gate.wait()                                                       # both threads have set theirs
+        seen[value] = binding.idg_get_option(binding.IDG_OPT_FUSE)
+        gate.wait()
+
+    ts = [threading.Thread(target=worker, args=(v,)) for v in (2, 4)]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join()
+    assert seen == {2: 2, 4: 4}
+    assert binding.idg_get_option(binding.IDG_OPT_FUSE) == 1
+    binding.idg_set_option(binding.IDG_OPT_FUSE, 0)
+
+
+def test_stats_rms(binding):
+    """idg_stats_rms: mean and sqrt(<x^2> - <x>^2) from (n, sum, sum of squares); against numpy on a small sample."""
+    import numpy as np
+    x = np.random.default_rng(3).normal(2.0, 1.5, 1000)
+    mean, rms = binding.idg_stats_rms([x.size, x.sum(), (x * x).sum()])
+    assert mean == pytest.approx(x.mean(), rel=1e-12) and rms == pytest.approx(x.std(), rel=1e-10)
+    assert all(np.isnan(v) for v in binding.idg_stats_rms([0.0, 0.0, 0.0]))
+
+
+def test_resident_shapes_reserve_mailboxes(binding):
+    """Cubes the resident kernel can take (nx % 4 == 0, <= 4 Mi voxels) carry 32 MB of mailboxes in the workspace."""
+    small = binding.idg_workspace_bytes(100, 100, 67, 1)
+    assert small >= 100 * 100 * 67 * 4 + (32 << 20)
+    assert binding.idg_workspace_bytes(102, 100, 67, 1) < 102 * 100 * 67 * 4 + (1 << 20)        # nx % 4 != 0
+    assert binding.idg_workspace_bytes(1024, 1024, 512, 1) < 1024 * 1024 * 512 * 4 + (1 << 20)  # too large
 
 
 def test_cpu_tensor_is_rejected(binding):

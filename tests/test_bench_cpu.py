@@ -70,11 +70,17 @@ def test_reference_arm_under_torchrun_world2():
     assert r["e2e"] == {"value": r["value"], "unit": r["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
 
 
-def test_traffic_table_lookup():
-    """bench.py's `roofline.traffic` comes from profiles/traffic.txt, keyed by "<plan> <workload>"; the plan
-    string itself contains '=' signs."""
+def test_ncu_counter_table_lookup():
+    """bench.py's `roofline.traffic`, its ALU figures and L2 bytes come from profiles/ncu_per_launch.json, keyed by
+    (plan, workload); every entry names the note and commit it was measured at, and a plan that was never captured
+    on a workload gets nothing (the line then withholds the figures instead of borrowing another plan's)."""
     sys.path.insert(0, ROOT)
     import bench
-    v = bench.ncu_traffic_bytes("idg_tma_kernel fuse=4 tile=0 cfg3_1024x1024x512_n20")
-    assert v is not None and 4.2e9 < v < 4.6e9          # one read + one write of the 2.147 GB cube, plus halo
-    assert bench.ncu_traffic_bytes("no such kernel cfg3_1024x1024x512_n20") is None
+    e = bench.ncu_counters("idg_tma_kernel fuse=4 tile=0", "cfg3_1024x1024x512_n20")
+    assert 4.2e9 < e["dram_bytes"] < 4.6e9 and e["warp_instructions"] > 9e8 and "source" in e and "commit" in e
+    assert bench.ncu_counters("no such kernel", "cfg3_1024x1024x512_n20") == {}
+    assert bench.ncu_counters("idg_tma_kernel fuse=4 tile=0", "cfg0_100x100x67_n10") == {}
+    table = json.load(open(os.path.join(ROOT, "profiles", "ncu_per_launch.json")))["entries"]
+    for entry in table:
+        assert os.path.exists(os.path.join(ROOT, entry["source"].split(" ")[0])), entry["source"]
+        assert entry["workload"] in bench.WORKLOADS

@@ -28,10 +28,8 @@ def B():
 
 
 # (kernel, fuse) plans every parity case runs under
-PLANS = [(1, 0), (2, 1), (2, 2), (2, 3), (2, 4), (3, 1), (3, 2), (3, 3), (3, 4),
-         (4, 1), (4, 2), (4, 3), (4, 4), (5, 0), (0, 0)]
-PLAN_IDS = ["naive", "tiled-T1", "tiled-T2", "tiled-T3", "tiled-T4", "tma-T1", "tma-T2", "tma-T3", "tma-T4",
-            "stream-T1", "stream-T2", "stream-T3", "stream-T4", "resident", "auto"]
+PLANS = [(1, 0), (2, 1), (2, 2), (2, 4), (3, 1), (3, 2), (3, 3), (3, 4), (5, 0), (0, 0)]
+PLAN_IDS = ["naive", "tiled-T1", "tiled-T2", "tiled-T4", "tma-T1", "tma-T2", "tma-T3", "tma-T4", "resident", "auto"]
 
 
 def set_plan(B, plan, zchunk=0, tile=0, ctas=0, coop=None):
@@ -114,19 +112,6 @@ def test_tma_tile_variants(B, oracle, fuse, tile):
     c = synth.modelb_like(seed=1000, snr=32.0)
     p = B.Params()
     assert err(gpu(B, c.data, 10, p), oracle.idg_filter_oracle(c.data, 10, **p.f32()), c.rms) <= TOL
-
-
-@pytest.mark.parametrize("ctas", [1, 2, 7, 61, 148, 1000])
-@pytest.mark.parametrize("tile", [1, 2])
-@pytest.mark.parametrize("fuse", [1, 2, 3, 4])
-def test_stream_grid_variants(B, oracle, fuse, tile, ctas):
-    """Persistent kernel: any split of the tile-plane stream over CTAs (segments that start and end
-    mid-tile, one CTA walking over all tiles, more CTAs than planes) gives the same cube."""
-    set_plan(B, (4, fuse), 0, tile, ctas)
-    rng = np.random.default_rng(23)
-    a = rng.normal(0, 2, (13, 150, 268)).astype(np.float32)
-    p = B.Params(K=1.0, tau=0.03, cx=4.0, cy=5.0, cz=6.0, rms=2.0)
-    assert err(gpu(B, a, 7, p), oracle.idg_filter_oracle(a, 7, **p.f32()), 2.0) <= TOL
 
 
 def test_config1_parameter_sweep(B, oracle, parity_log):
@@ -558,7 +543,7 @@ def test_resident_kernel_is_bitwise_equal_to_the_naive_kernel_and_repeatable(B, 
     assert torch.equal(B.idg_filter_pm(x[0], 5, ps[0]), ref) and "idg_resident_kernel pm" in B.idg_last_plan()
 
 
-@pytest.mark.parametrize("plan", [(2, 2), (3, 1), (3, 2), (3, 3), (3, 4), (4, 1), (4, 2), (4, 3), (4, 4)],
+@pytest.mark.parametrize("plan", [(2, 2), (3, 1), (3, 2), (3, 3), (3, 4)],
                          ids=lambda p: f"k{p[0]}-T{p[1]}")
 def test_fused_kernels_are_bitwise_equal_to_the_naive_kernel_and_repeatable(B, plan):
     """Every kernel applies the same fp32 operations in the same order per voxel (packed fp32x2
@@ -570,7 +555,7 @@ def test_fused_kernels_are_bitwise_equal_to_the_naive_kernel_and_repeatable(B, p
     p = B.Params(K=1.5, tau=0.03, cx=5.0, cy=4.0, cz=6.0, rms=1.0)
     set_plan(B, (1, 0))
     ref = B.idg_filter(x, 7, p)
-    for tile in ((1, 2) if plan[0] >= 3 and plan[1] <= 2 else ((0, 3) if plan[0] == 3 else (0,))):
+    for tile in ((1, 2) if plan[0] == 3 and plan[1] <= 2 else ((0, 3) if plan[0] == 3 else (0,))):
         for rep in range(4):
             set_plan(B, plan, 0, tile)
             out = B.idg_filter(x, 7, p)

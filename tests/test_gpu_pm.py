@@ -25,7 +25,7 @@ def plan(B, kernel, fuse, tile):
     B.idg_set_option(B.IDG_OPT_TILE, tile)
 
 
-PLANS = [(1, 0, 0), (4, 1, 1), (4, 1, 2), (4, 2, 1), (4, 2, 2), (3, 1, 0), (3, 2, 0), (3, 3, 0), (3, 4, 0), (0, 0, 0)]
+PLANS = [(1, 0, 0), (3, 1, 0), (3, 2, 0), (3, 3, 0), (3, 4, 0), (5, 0, 0), (0, 0, 0)]
 SHAPES = [(1, 1, 1), (4, 4, 4), (7, 6, 5), (3, 5, 8), (2, 3, 260), (9, 70, 132), (21, 67, 100), (13, 150, 268)]
 
 
@@ -57,9 +57,9 @@ def test_pm_config0_and_invariants(B, oracle):
     assert torch.equal(B.idg_filter_pm(t, 6, lin), B.idg_filter(t, 6, lin))
     k = torch.full((10, 40, 64), 3.25, device="cuda")
     assert float((B.idg_filter_pm(k, 9, B.Params()) - k).abs().max()) <= 3.25 * 9 * 2.0 ** -23   # fixed point to rounding
-    # fused kernels (persistent kernel 4, TMA kernel 3 at every depth, auto plan) == naive kernel, bit for bit
+    # fused kernels (TMA kernel 3 at every depth, resident kernel 5, auto plan) == naive kernel, bit for bit
     plan(B, 1, 0, 0)
     ref = B.idg_filter_pm(t, 7, B.Params())
-    for p in ((4, 1, 1), (4, 2, 1), (4, 2, 2), (3, 1, 0), (3, 2, 0), (3, 3, 0), (3, 4, 0), (0, 0, 0)):
+    for p in ((3, 1, 0), (3, 2, 0), (3, 3, 0), (3, 4, 0), (5, 0, 0), (0, 0, 0)):
         plan(B, *p)
         assert torch.equal(B.idg_filter_pm(t, 7, B.Params()), ref), p

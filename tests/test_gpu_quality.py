@@ -65,7 +65,7 @@ def test_quality_on_a_filtered_config0_cube(B, Q, oracle):
     st = B.idg_cube_stats(filt, (0, 100, 0, 100, 0, 8)).cpu().numpy()      # signal-free channels
     ref = Q.cube_stats_oracle(filt.cpu().numpy(), (0, 100, 0, 100, 0, 8))
     assert st[0] == ref["n"] and abs(st[1] - ref["sum"]) <= 1e-9 and abs(st[2] - ref["sumsq"]) <= 1e-9
-    rms_f = math.sqrt(st[2] / st[0] - (st[1] / st[0]) ** 2)
+    rms_f = B.idg_stats_rms(st)[1]
     assert rms_f == pytest.approx(ref["rms"], rel=1e-9) and rms_f < 0.7 * c.rms    # the filter lowers the noise
     model = torch.from_numpy(c.model).cuda() if getattr(c, "model", None) is not None else None
     roi = (10, 90, 10, 90, 10, 60)

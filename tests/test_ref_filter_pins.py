@@ -160,6 +160,8 @@ def test_g5_second_moments_rotate_with_the_kernel(oracle):
 
 def test_g6_constant_cube_and_impulse(oracle):
     a = np.full((5, 6, 7), -1.5)
+    # 1e-13, not 1e-15: the direct sum adds 343 fp64 products (r = 3) of unit-sum weights, which do not add up to exactly 1; its
+    # rounding (summation order, a few tens of ulp of 1.5) is a few 1e-15..1e-14 -- a property of fp64 summation, not of the filter
     assert np.abs(oracle.gaussian_filter_oracle(a, (3, 3, 3)) - a).max() < 1e-13
     a = np.zeros((21, 21, 21))
     a[10, 10, 10] = 3.0
@@ -168,7 +170,7 @@ def test_g6_constant_cube_and_impulse(oracle):
         out = oracle.gaussian_filter_oracle(a, (5, 3, 2), theta)
         rz, ry, rx = (n // 2 for n in k.shape)
         got = out[10 - rz:11 + rz, 10 - ry:11 + ry, 10 - rx:11 + rx]
-        assert np.abs(got - 3.0 * k).max() < 1e-14                 # the impulse response is the kernel
+        assert np.abs(got - 3.0 * k).max() < 1e-14                 # the impulse response is the kernel (3.0 * k rounds once more than the oracle's sum of one non-zero term: a few ulp of 0.1)
         assert abs(out.sum() - 3.0) < 1e-13
 
 
