@@ -35,6 +35,12 @@ bool voxel_count(int nx, int ny, int nz, int batch, size_t *n_one)
 // workspace then carries the mailbox region.
 bool resident_shape(int nx, size_t N) { return nx % 4 == 0 && N <= idg::kResidentMaxCubeVoxels; }
 
+// Bytes of one pitched copy of a batch (row pitch = nx rounded up to a multiple of 4 floats = 16 bytes).
+size_t pitched_bytes(int nx, int ny, int nz, int batch)
+{
+    return (size_t)((nx + 3) / 4 * 4) * (size_t)ny * (size_t)nz * (size_t)batch * sizeof(float);
+}
+
 bool params_valid(const idg_params &p)
 {
     if (!(p.K > 0.0f)) return false;                         // rejects NaN, 0, negatives; +inf passes
@@ -90,7 +96,8 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
         return IDG_ERR_OVERLAP;
 
     float *scratch = (float *)workspace;
-    idg::CubeParams *tab = (idg::CubeParams *)((char *)workspace + align_up(bytes));
+    const size_t pbytes = pitched_bytes(nx, ny, nz, batch);
+    idg::CubeParams *tab = (idg::CubeParams *)((char *)workspace + align_up(nx % 4 ? 3 * pbytes : bytes));
     unsigned *coop_bar = (unsigned *)((char *)tab + align_up(sizeof(idg::CubeParams) * (size_t)batch));
     unsigned long long *mail = (unsigned long long *)((char *)coop_bar + kAlign);
     const size_t mail_bytes = resident_shape(nx, N) ? idg::kResidentMailBytes : 0;
@@ -101,6 +108,9 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     int kernel = g_opt[IDG_OPT_KERNEL];
     int fuse = g_opt[IDG_OPT_FUSE];
     int tile = g_opt[IDG_OPT_TILE];
+    // nx % 4 != 0: kernel 3 on the library's pitched copies in the workspace (intensity-driven filter only)
+    const bool pitched_ok = mode == 0 && idg::tma_pitched_supported(nx, ny, nz);
+    bool pitched = false;
     // Small cubes and interactive batches: everything on chip for the whole call (profiles/r2a_notes.md).
     idg::ResidentPlan rplan;
     const bool can_resident = mail_bytes > 0 && max_n > 0 && (((uintptr_t)cubes | (uintptr_t)out) & 15u) == 0 &&
@@ -124,10 +134,15 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
             // (profiles/r1k_notes.md).
             if (!fuse && work <= kCoopMaxVoxels && g_opt[IDG_OPT_COOP] != 1 && max_n >= 5) fuse = 3;
             if (!fuse) fuse = (nz < 100 && work >= 4.0e6) ? 2 : 4;
+        } else if (pitched_ok && (double)N * (double)batch >= 1.0e5) {
+            kernel = 3;                        // on pitched copies (profiles/r2c_notes.md)
+            pitched = true;
+            if (!fuse) fuse = (nz < 100 && work >= 4.0e6) ? 2 : 4;
         } else {
             kernel = can_tile ? 2 : 1;
         }
     }
+    if (g_opt[IDG_OPT_KERNEL] == 3 && !can_tma && pitched_ok) pitched = true;
     if (mode == 1 && kernel != 5) {          // gradient-driven variant: kernel 3 (any T) or the naive kernel
         const int ko = g_opt[IDG_OPT_KERNEL];
         fuse = g_opt[IDG_OPT_FUSE];
@@ -139,7 +154,8 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
         }
     }
     if (kernel == 4) kernel = can_tma ? 3 : 2;      // kernel 4 (persistent warp-decoupled variant) was retired in 1.1
-    if (kernel == 3 && !can_tma) kernel = 2;
+    if (kernel == 3 && !can_tma && !pitched) kernel = 2;
+    if (kernel != 3) pitched = false;
     if (kernel == 2 && !can_tile) kernel = 1;
     if (kernel == 5) {
         fuse = max_n;
@@ -152,7 +168,8 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     {
         static const char *const names[6] = {"", "idg_naive_kernel", "idg_tiled_kernel", "idg_tma_kernel",
                                              "", "idg_resident_kernel"};
-        snprintf(t_plan, sizeof(t_plan), "%s%s fuse=%d tile=%d", names[kernel], mode == 1 ? " pm" : "", fuse, tile);
+        snprintf(t_plan, sizeof(t_plan), "%s%s%s fuse=%d tile=%d", names[kernel], mode == 1 ? " pm" : "",
+                 pitched ? " pitched" : "", fuse, tile);
     }
 
     std::vector<idg::CubeParams> host_tab((size_t)batch);
@@ -209,7 +226,18 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
         }
         return (int)e;
     }
-    if (in_place) {     // stage I_0 so a cube whose first launch targets `out` does not read what it writes
+    if (pitched) {      // dense -> pitched input copy; the launches ping-pong between the other two pitched buffers
+        const int pitch = (nx + 3) / 4 * 4;
+        float *p0 = scratch, *p1 = (float *)((char *)scratch + pbytes), *p2 = (float *)((char *)scratch + 2 * pbytes);
+        e = idg::launch_repitch(cubes, nx, p0, pitch, nullptr, nullptr, nx, ny, nz, batch, st);
+        if (e != cudaSuccess) return (int)e;
+        ++t_launches;
+        L.in = p0;
+        L.out = p1;
+        L.scratch = p2;
+        L.pitch = pitch;
+        L.in_place = 0;
+    } else if (in_place) {     // stage I_0 so a cube whose first launch targets `out` does not read what it writes
         e = cudaMemcpyAsync(scratch, cubes, bytes, cudaMemcpyDeviceToDevice, st);
         if (e != cudaSuccess) return (int)e;
     }
@@ -217,7 +245,7 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     // grid is co-resident.  Measured on B200 (profiles/r1k_notes.md).
     const int rounds = (max_n + fuse - 1) / fuse;
     const int coop = g_opt[IDG_OPT_COOP];
-    if (kernel == 3 && mode == 0 && rounds >= 2 && coop != 1 &&
+    if (kernel == 3 && mode == 0 && !pitched && rounds >= 2 && coop != 1 &&
         (coop == 2 || (double)N * (double)batch <= kCoopMaxVoxels)) {
         e = cudaMemsetAsync(coop_bar, 0, 8, st);
         if (e != cudaSuccess) return (int)e;
@@ -245,6 +273,11 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
         e = (kernel == 3)   ? idg::launch_tma(L, g_opt[IDG_OPT_ZCHUNK], tile_now, st)
             : (kernel == 2) ? idg::launch_tiled(L, g_opt[IDG_OPT_ZCHUNK], st)
                             : idg::launch_naive(L, st);
+        if (e != cudaSuccess) return (int)e;
+        ++t_launches;
+    }
+    if (pitched) {      // pitched result -> the caller's dense cubes (cubes with n_iter = 0: their input copy)
+        e = idg::launch_repitch(L.out, L.pitch, out, nx, L.in, L.tab, nx, ny, nz, batch, st);
         if (e != cudaSuccess) return (int)e;
         ++t_launches;
     }
@@ -287,7 +320,9 @@ size_t idg_workspace_bytes(int nx, int ny, int nz, int batch)
 {
     size_t N;
     if (!voxel_count(nx, ny, nz, batch, &N)) return 0;
-    return align_up(N * (size_t)batch * sizeof(float)) + align_up(sizeof(idg::CubeParams) * (size_t)batch) +
+    // nx % 4 != 0: three pitched copies of the batch (input, and the two ping-pong buffers) instead of one scratch
+    const size_t cubes = nx % 4 ? 3 * pitched_bytes(nx, ny, nz, batch) : N * (size_t)batch * sizeof(float);
+    return align_up(cubes) + align_up(sizeof(idg::CubeParams) * (size_t)batch) +
            kAlign +     // scratch cubes | per-cube constants | arrival counter of the cooperative launch
            (resident_shape(nx, N) ? idg::kResidentMailBytes : 0);      // | mailboxes of the resident kernel
 }

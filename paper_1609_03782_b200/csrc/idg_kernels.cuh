@@ -32,7 +32,15 @@ struct Launch {
     int fuse;               // iterations per launch of this plan (T)
     int in_place;           // out == in: the host staged a copy of I_0 in `scratch`
     int mode;               // 0: intensity-driven conductance (Eq. 6); 1: gradient-driven (Eq. 5, idg_filter_pm)
+    int pitch;              // row pitch in floats of the three buffers; 0 = dense (nx).  > nx: the library's own
+                            // pitched copies of cubes with nx % 4 != 0 (kernel 3 only)
 };
+
+// floats from one cube of a batch to the next
+__host__ __device__ __forceinline__ size_t cube_stride(const Launch &L)
+{
+    return (size_t)(L.pitch ? L.pitch : L.nx) * (size_t)L.ny * (size_t)L.nz;
+}
 
 // Which buffers cube b reads / writes in this launch so that its LAST launch writes `out`.
 // Returns the number of iterations to apply now (0 = cube already finished).
@@ -44,7 +52,7 @@ __device__ __forceinline__ int route(const Launch &L, int iter_done, int b, cons
     if (remaining <= 0) return 0;
     const int now = remaining < L.fuse ? remaining : L.fuse;
     const int after = (remaining - now + L.fuse - 1) / L.fuse;      // launches still to come
-    const size_t off = (size_t)b * (size_t)L.nx * (size_t)L.ny * (size_t)L.nz;
+    const size_t off = (size_t)b * cube_stride(L);
     float *o = L.out + off, *s = L.scratch + off;
     dst = (after & 1) ? s : o;
     if (iter_done == 0)     // first launch: read I_0 (from the staged copy if it would alias dst)
@@ -105,6 +113,11 @@ cudaError_t launch_naive(const Launch &L, cudaStream_t st);
 cudaError_t launch_tiled(const Launch &L, int zchunk, cudaStream_t st);
 bool tiled_supported(int nx, int ny, int nz, const void *in, const void *out, const void *scratch);
 cudaError_t launch_tma(const Launch &L, int zchunk, int tile, cudaStream_t st);
+// Cubes with nx % 4 != 0 run kernel 3 on pitched copies (row pitch = nx rounded up to 4 floats): dense -> pitched
+// before the first launch, pitched -> dense after the last (cubes with n_iter = 0 take their input copy).
+bool tma_pitched_supported(int nx, int ny, int nz);
+cudaError_t launch_repitch(const float *src, int src_pitch, float *dst, int dst_pitch, const float *src_zero,
+                           const CubeParams *tab, int nx, int ny, int nz, int batch, cudaStream_t st);
 // All `rounds` launches of a plan (fuse iterations each) as ONE cooperative launch with grid barriers in between, for
 // workloads whose whole grid is co-resident (small, L2-resident cubes).  bar: 8 zeroed bytes of device memory.
 // cudaErrorNotSupported / cudaErrorCooperativeLaunchTooLarge: use launch_tma per round instead.
@@ -145,7 +158,7 @@ cudaError_t temp_trim();
 // Tensor maps for the TMA kernels (idg_tmap.cu): 4-D (x, y, z, cube), box tile_x x tile_y x 1 x 1, zero fill.
 bool tmap_available();
 bool tmap_encode(CUtensorMap *m, const float *base, int nx, int ny, int nz, int batch, int tile_x, int tile_y,
-                 int tile_z = 1);
+                 int tile_z = 1, int pitch = 0);
 
 // Reference filters (PAPER.md sections 3.1-3.2): separable single-pass filter (box, axis-aligned
 // Gaussian) and dense 3-D convolution (rotated Gaussian, Eq. 3).

@@ -63,7 +63,9 @@ struct Smem {
 
 // ONE: the cube has at most 128 columns, so a single tile column covers a row with all 32 lanes valid and no halo
 // lanes; the x faces are replicated by patching the shuffled neighbour of the first / last float4 of the row.
-template <int TL, int R, int WARPS, int NS, int TMAX, bool ONE, bool PM = false>
+// UNAL: nx % 4 != 0 -- the buffers are pitched copies (row pitch L.pitch), the x face at nx - 1 lies INSIDE a float4:
+// cells beyond it take the even reflection element by element (cell x <- cell 2 nx - 1 - x) from the level-0 stage.
+template <int TL, int R, int WARPS, int NS, int TMAX, bool ONE, bool PM = false, bool UNAL = false>
 __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restrict__ dst, const Launch &L,
                                          const TmaArgs &A, const CubeParams &prm, int b,
                                          unsigned char *smem, bool reinit = false)
@@ -76,7 +78,8 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
 
     const int lane = threadIdx.x & 31;
     const int wy = threadIdx.x >> 5;
-    const int nx4 = L.nx >> 2;
+    const int nx4 = UNAL ? (L.nx + 3) >> 2 : L.nx >> 2;       // float4 columns that hold cube voxels
+    const int ld = UNAL ? L.pitch : L.nx;                      // row pitch of the buffers
     const int vy = TILE_Y - 2 * A.halo;
     const int ti = blockIdx.x % A.tiles_x, tj = blockIdx.x / A.tiles_x;
     const int tx0 = ONE ? 0 : (ti * kValidLanes - 1) * 4;   // cube x of tile column 0
@@ -93,9 +96,12 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
     unsigned ok = 0, fix = 0;
     bool rev = false;
     int slane = lane;
+    // UNAL: tile column of the first cell beyond the x face, and the sum of a cell's and its mirror image's columns
+    const int xw = UNAL ? L.nx - tx0 : 0, xc = 2 * xw - 1;
+    const bool xfix = UNAL && lane * 4 + 3 >= xw;              // some component of my float4 lies beyond the face
     if (!ONE) {
         if (x4 < 0) { slane = lane + (-1 - x4) - x4; rev = true; }             // x4' = -1 - x4
-        else if (x4 >= nx4) { slane = lane + (2 * nx4 - 1 - x4) - x4; rev = true; }
+        else if (!UNAL && x4 >= nx4) { slane = lane + (2 * nx4 - 1 - x4) - x4; rev = true; }
         if (slane < 0 || slane >= kLanes) { slane = lane; rev = false; }        // beyond one reflection: unused cell
     }
 #pragma unroll
@@ -107,7 +113,7 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
         else if (gy >= L.ny) srow = (2 * L.ny - 1 - gy) - ty0;
         if (srow < 0 || srow >= TILE_Y) srow = row;
         scell[r] = srow * kTileX + slane * 4;
-        if (scell[r] != cell[r]) fix |= 1u << r;
+        if (scell[r] != cell[r] || xfix) fix |= 1u << r;
         if ((ONE || (lane >= 1 && lane <= kValidLanes)) && x4 < nx4 && row >= A.halo && row < TILE_Y - A.halo &&
             gy < L.ny)
             ok |= 1u << r;
@@ -116,8 +122,8 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
     const int dn_cell = min(row0 + R, TILE_Y - 1) * kTileX + lane * 4;
     const int wy_up = max(wy - 1, 0), wy_dn = min(wy + 1, WARPS - 1);
 
-    const size_t plane = (size_t)L.nx * (size_t)L.ny;
-    float *po = dst + (long long)(ty0 + row0) * L.nx + (long long)x4 * 4 + (long long)(q_first - TL - 1) * (long long)plane;
+    const size_t plane = (size_t)ld * (size_t)L.ny;
+    float *po = dst + (long long)(ty0 + row0) * ld + (long long)x4 * 4 + (long long)(q_first - TL - 1) * (long long)plane;
 
     if (threadIdx.x == 0) {
 #pragma unroll
@@ -176,6 +182,14 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
             for (int r = 0; r < R; ++r)
                 if (fix & (1u << r)) {
                     if (rev) nw[0][r] = F4{nw[0][r].w, nw[0][r].z, nw[0][r].y, nw[0][r].x};
+                    if (UNAL && xfix) {      // beyond the x face: the mirror image, component by component
+                        const float *row = st + (scell[r] - slane * 4);
+                        const int c0 = lane * 4;
+                        if (c0 >= xw) nw[0][r].x = row[min(max(xc - c0, 0), kTileX - 1)];
+                        if (c0 + 1 >= xw) nw[0][r].y = row[min(max(xc - c0 - 1, 0), kTileX - 1)];
+                        if (c0 + 2 >= xw) nw[0][r].z = row[min(max(xc - c0 - 2, 0), kTileX - 1)];
+                        if (c0 + 3 >= xw) nw[0][r].w = row[min(max(xc - c0 - 3, 0), kTileX - 1)];
+                    }
                     sts4(const_cast<float *>(st) + cell[r], nw[0][r]);
                 }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // the stage is refilled by TMA later on
@@ -221,7 +235,7 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
 #pragma unroll
             for (int r = 0; r < R; ++r)
                 if (ok & (1u << r))
-                    *reinterpret_cast<float4 *>(po + (long long)r * L.nx) =
+                    *reinterpret_cast<float4 *>(po + (long long)r * ld) =
                         make_float4(out[r].x, out[r].y, out[r].z, out[r].w);
         }
         par ^= 1;
@@ -239,7 +253,7 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
     }
 }
 
-template <int T, int R, int WARPS, int NS, int MINB, bool ONE, bool PM = false>
+template <int T, int R, int WARPS, int NS, int MINB, bool ONE, bool PM = false, bool UNAL = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 idg_tma_kernel(const __grid_constant__ Launch L, const __grid_constant__ TmaArgs A,
                const __grid_constant__ Maps M)
@@ -251,12 +265,12 @@ idg_tma_kernel(const __grid_constant__ Launch L, const __grid_constant__ TmaArgs
     float *dst;
     const int now = route(L, b, prm, src, dst);
     if (now == 0) return;
-    const size_t off = (size_t)b * (size_t)L.nx * (size_t)L.ny * (size_t)L.nz;
+    const size_t off = (size_t)b * cube_stride(L);
     const CUtensorMap *map = (src == L.scratch + off) ? &M.scratch : (src == L.out + off) ? &M.out : &M.in;
-    if (now == T) tma_body<T, R, WARPS, NS, T, ONE, PM>(map, dst, L, A, prm, b, smem);
-    else if (T > 1 && now == 1) tma_body<1, R, WARPS, NS, T, ONE, PM>(map, dst, L, A, prm, b, smem);
-    else if (T > 2 && now == 2) tma_body<(T > 2 ? 2 : 1), R, WARPS, NS, T, ONE, PM>(map, dst, L, A, prm, b, smem);
-    else if (T > 3 && now == 3) tma_body<(T > 3 ? 3 : 1), R, WARPS, NS, T, ONE, PM>(map, dst, L, A, prm, b, smem);
+    if (now == T) tma_body<T, R, WARPS, NS, T, ONE, PM, UNAL>(map, dst, L, A, prm, b, smem);
+    else if (T > 1 && now == 1) tma_body<1, R, WARPS, NS, T, ONE, PM, UNAL>(map, dst, L, A, prm, b, smem);
+    else if (T > 2 && now == 2) tma_body<(T > 2 ? 2 : 1), R, WARPS, NS, T, ONE, PM, UNAL>(map, dst, L, A, prm, b, smem);
+    else if (T > 3 && now == 3) tma_body<(T > 3 ? 3 : 1), R, WARPS, NS, T, ONE, PM, UNAL>(map, dst, L, A, prm, b, smem);
 }
 
 // Cooperative variant: all `A.rounds` launches of a plan in one, a grid barrier between rounds (the whole grid is
@@ -269,7 +283,7 @@ idg_tma_coop_kernel(const __grid_constant__ Launch L, const __grid_constant__ Tm
     extern __shared__ __align__(1024) unsigned char smem[];
     const int b = blockIdx.z;
     const CubeParams prm = cube_params(L, b);
-    const size_t off = (size_t)b * (size_t)L.nx * (size_t)L.ny * (size_t)L.nz;
+    const size_t off = (size_t)b * cube_stride(L);
     constexpr bool COOP = true;
     const int rounds = A.rounds;
     const unsigned ctas = gridDim.x * gridDim.y * gridDim.z;
@@ -293,7 +307,7 @@ idg_tma_coop_kernel(const __grid_constant__ Launch L, const __grid_constant__ Tm
 
 bool encode_map(CUtensorMap *m, const float *base, const Launch &L, int tile_y)
 {
-    return tmap_encode(m, base, L.nx, L.ny, L.nz, L.batch, kTileX, tile_y);
+    return tmap_encode(m, base, L.nx, L.ny, L.nz, L.batch, kTileX, tile_y, 1, L.pitch);
 }
 
 // max_ctas > 0: only chunkings whose whole grid is at most max_ctas CTAs (cooperative launch); 0 if none is.
@@ -329,17 +343,20 @@ cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st, int rounds 
     A.halo = T;
     A.rounds = rounds;
     A.bar = bar;
-    const bool one = L.nx <= kTileX;                     // a single tile column: no halo lanes
-    A.tiles_x = one ? 1 : (L.nx / 4 + kValidLanes - 1) / kValidLanes;
+    const bool unal = L.pitch > 0;                       // nx % 4 != 0: pitched buffers, the face inside a float4
+    const bool one = L.nx <= kTileX && !unal;            // a single tile column: no halo lanes
+    A.tiles_x = one ? 1 : ((L.nx + 3) / 4 + kValidLanes - 1) / kValidLanes;
     A.tiles_y = (L.ny + (TILE_Y - 2 * T) - 1) / (TILE_Y - 2 * T);
     const long tiles = (long)A.tiles_x * A.tiles_y;
     if (tiles > 0x7fffffffL) return cudaErrorInvalidValue;
     void (*kern)(Launch, TmaArgs, Maps);
     if constexpr (COOP) kern = one ? idg_tma_coop_kernel<T, R, WARPS, NS, MINB, true> : idg_tma_coop_kernel<T, R, WARPS, NS, MINB, false>;
+    else if (unal && !PM) kern = idg_tma_kernel<T, R, WARPS, NS, MINB, false, false, !PM>;      // (!PM: no pm instantiation)
     else kern = one ? idg_tma_kernel<T, R, WARPS, NS, MINB, true, PM> : idg_tma_kernel<T, R, WARPS, NS, MINB, false, PM>;
-    static DeviceOnce smem_once[2];
+    if (unal && (COOP || PM)) return cudaErrorNotSupported;
+    static DeviceOnce smem_once[3];
     {
-        const cudaError_t e = set_max_dynamic_smem(smem_once[one], (const void *)kern, S::kBytes);
+        const cudaError_t e = set_max_dynamic_smem(smem_once[unal ? 2 : one], (const void *)kern, S::kBytes);
         if (e != cudaSuccess) return e;
     }
     const int sms = device_sm_count();
@@ -381,6 +398,41 @@ bool tma_supported(int nx, int ny, int nz, const void *in, const void *out, cons
     const uintptr_t m = (uintptr_t)in | (uintptr_t)out | (uintptr_t)scratch;
     if ((m & 15u) != 0) return false;
     return tmap_available();
+}
+
+bool tma_pitched_supported(int nx, int ny, int nz)
+{
+    (void)nz;
+    return nx % 4 != 0 && nx >= 5 && ny >= 4 && tmap_available();
+}
+
+namespace {
+// Row-by-row copy between a dense cube (pitch nx) and its pitched copy; cubes whose n_iter is 0 take src_zero
+// (their untouched input copy) instead of src.
+__global__ void idg_repitch_kernel(const float *__restrict__ src, int src_pitch, float *__restrict__ dst, int dst_pitch,
+                                   const float *__restrict__ src_zero, const CubeParams *__restrict__ tab, int nx,
+                                   size_t rows_per_cube, size_t rows)
+{
+    for (size_t row = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); row < rows;
+         row += (size_t)gridDim.x * (blockDim.x >> 5)) {
+        const float *s = src;
+        if (src_zero && tab && tab[row / rows_per_cube].n_iter == 0) s = src_zero;
+        const float *sr = s + row * (size_t)src_pitch;
+        float *dr = dst + row * (size_t)dst_pitch;
+        for (int x = threadIdx.x & 31; x < nx; x += 32) dr[x] = sr[x];
+    }
+}
+}  // namespace
+
+cudaError_t launch_repitch(const float *src, int src_pitch, float *dst, int dst_pitch, const float *src_zero,
+                           const CubeParams *tab, int nx, int ny, int nz, int batch, cudaStream_t st)
+{
+    const size_t rows_per_cube = (size_t)ny * (size_t)nz, rows = rows_per_cube * (size_t)batch;
+    size_t blocks = (rows + 7) / 8;
+    const size_t cap = (size_t)device_sm_count() * 32;
+    if (blocks > cap) blocks = cap;
+    idg_repitch_kernel<<<(unsigned)blocks, 256, 0, st>>>(src, src_pitch, dst, dst_pitch, src_zero, tab, nx, rows_per_cube, rows);
+    return cudaGetLastError();
 }
 
 // tile (T = fused iterations): T <= 2: 0, 1 = 128x64 tile, 512 threads, one CTA per SM | 2 = 128x32 tile, 256

@@ -111,13 +111,15 @@ cudaError_t temp_trim()
 
 bool tmap_available() { return encode_fn() != nullptr; }
 
+// pitch: row pitch in floats (0 = nx); elements nx .. pitch-1 of a row lie outside the tensor (zero fill)
 bool tmap_encode(CUtensorMap *m, const float *base, int nx, int ny, int nz, int batch, int tile_x, int tile_y,
-                 int tile_z)
+                 int tile_z, int pitch)
 {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
+    const cuuint64_t ld = (cuuint64_t)(pitch ? pitch : nx);
     const cuuint64_t dims[4] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz, (cuuint64_t)batch};
-    const cuuint64_t strides[3] = {(cuuint64_t)nx * 4, (cuuint64_t)nx * ny * 4, (cuuint64_t)nx * ny * (cuuint64_t)nz * 4};
+    const cuuint64_t strides[3] = {ld * 4, ld * ny * 4, ld * ny * (cuuint64_t)nz * 4};
     const cuuint32_t box[4] = {(cuuint32_t)tile_x, (cuuint32_t)tile_y, (cuuint32_t)tile_z, 1};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void *)base, dims, strides, box, estr,

@@ -543,6 +543,40 @@ def test_resident_kernel_is_bitwise_equal_to_the_naive_kernel_and_repeatable(B, 
     assert torch.equal(B.idg_filter_pm(x[0], 5, ps[0]), ref) and "idg_resident_kernel pm" in B.idg_last_plan()
 
 
+@pytest.mark.parametrize("nx", [5, 6, 7, 9, 33, 45, 101, 102, 103, 117, 121, 123, 127, 129, 250, 515])
+def test_unaligned_rows_run_the_tma_kernel_on_pitched_copies(B, oracle, nx):
+    """nx % 4 != 0 (real HI cubes rarely have nx % 4 = 0): kernel 3 runs on the library's pitched copies in the
+    workspace, the x face inside a float4 handled by element-wise reflection at level 0.  Bit-identical to the
+    one-thread-per-voxel kernel for every fusion depth, for batches with per-cube iteration counts (0 included), in
+    place; the auto plan takes this path from 1e5 voxels on."""
+    g = torch.Generator(device="cuda").manual_seed(nx)
+    ny, nz, nb = (37, 9, 3) if nx < 200 else (70, 11, 2)
+    x = torch.randn((nb, nz, ny, nx), device="cuda", generator=g) * 2.0
+    ps = [B.Params(K=1.0 + 0.5 * b, tau=0.03, cx=5.0, cy=4.0, cz=6.0, rms=1.0) for b in range(nb)]
+    ns = [7, 0, 10][:nb]
+    set_plan(B, (1, 0))
+    ref = B.idg_filter_batched(x, ns, ps)
+    ref1 = B.idg_filter(x[0], 9, ps[0])
+    for fuse in (1, 2, 3, 4):
+        set_plan(B, (3, fuse))
+        out = B.idg_filter_batched(x, ns, ps)
+        assert "pitched" in B.idg_last_plan(), B.idg_last_plan()
+        assert torch.equal(out, ref), (nx, fuse, int((out != ref).sum()))
+        inplace = x.clone()
+        B.idg_filter_batched(inplace, ns, ps, out=inplace)
+        assert torch.equal(inplace, ref)
+        assert torch.equal(B.idg_filter(x[0], 9, ps[0]), ref1)
+    set_plan(B, (0, 0))
+    big = torch.randn((40, 120, nx), device="cuda", generator=g)
+    if big.numel() >= 100_000:
+        out = B.idg_filter(big, 6, ps[0])
+        assert "pitched" in B.idg_last_plan()
+        set_plan(B, (1, 0))
+        assert torch.equal(out, B.idg_filter(big, 6, ps[0]))
+    want = oracle.idg_filter_oracle(x[0].cpu().numpy(), 9, **ps[0].f32())
+    assert err(ref1.cpu().numpy(), want, 1.0) <= TOL
+
+
 @pytest.mark.parametrize("plan", [(2, 2), (3, 1), (3, 2), (3, 3), (3, 4)],
                          ids=lambda p: f"k{p[0]}-T{p[1]}")
 def test_fused_kernels_are_bitwise_equal_to_the_naive_kernel_and_repeatable(B, plan):
