@@ -81,7 +81,9 @@ unsigned idg_params_check(const idg_params *params /*[host]*/);
 /*
  * Bytes of device workspace idg_filter_ws / idg_filter_batched need for `batch`
  * cubes of nx*ny*nz voxels: one scratch cube per cube (the "temporary eta" of
- * PAPER.md:430) plus a small parameter table, the 256-byte block holding the
+ * PAPER.md:430; for nx % 4 != 0 instead three copies of the batch with the row
+ * pitch rounded up to 16 bytes, on which the TMA-fed kernel runs) plus a small
+ * parameter table, the 256-byte block holding the
  * arrival counter of the cooperative single-launch path and, for cubes the resident
  * kernel can take (nx % 4 == 0, at most 4 Mi voxels), 32 MB of mailboxes for the
  * block faces.  0 on invalid dimensions.  A batch of more than ~2000 cubes uploads
