@@ -286,7 +286,9 @@ int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, i
  *   IDG_OPT_ZCHUNK   0 auto | >0  = planes per CTA along z (kernels 2, 3)
  *   IDG_OPT_TILE     0 auto | kernel 3: 1 = one CTA per SM (T <= 2: 128x64 tile, 512 threads; T >= 3: 128x32
  *                    tile, 256 threads), 2 = 128x32 tile, two 256-thread CTAs per SM (T <= 2), 3 = 384-thread CTA
- *                    (T >= 3) | separable reference filters: 2 = strips of 4
+ *                    (T >= 3), 4 = cluster pairs (T >= 3): two 256-thread CTAs stacked along y share a 128x64 tile and
+ *                    exchange their seam rows through distributed shared memory (measured slower than 1 at T = 4,
+ *                    faster at T = 3: profiles/r2b_notes.md) | separable reference filters: 2 = strips of 4
  *                    rows per thread instead of 2 in idg_sep3d_tma_kernel
  *   IDG_OPT_CTAS     reserved (was the grid size of the retired kernel 4); ignored
  *   IDG_OPT_HOST_SLABS  0 auto | 1..16 = z slabs of the idg_filter_host transfer/compute pipeline (1 = one piece)

@@ -69,6 +69,16 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
         "DONE_%=:\n\t}" ::"r"(bar), "r"(parity), "r"(0x989680)   // suspend-time hint: sleep, do not spin
         : "memory");
 }
+// Non-blocking: has the phase with the given parity completed?
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
 // As mbar_wait, without the suspend-time hint (plain try_wait loop).
 __device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity)
 {
@@ -109,6 +119,16 @@ __device__ __forceinline__ void grid_barrier(unsigned *bar, unsigned target)
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
+}
+// Split barrier over the CTAs of a cluster (all threads of all its CTAs): arrive releases this thread's shared-memory
+// traffic (its own CTA's and the partner's, through st.shared::cluster), wait acquires everybody else's.
+__device__ __forceinline__ void cluster_arrive()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void cluster_wait()
+{
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 __device__ __forceinline__ void sts32(uint32_t addr, uint32_t v)
 {

@@ -51,27 +51,41 @@ struct Maps {
     CUtensorMap in, out, scratch;      // the three cubes (batch as 4th dimension) a launch may read
 };
 
-template <int T, int R, int WARPS, int NS>
+// CL: two CTAs of a cluster share a tile of 2 TILE_Y rows (see tma_body): a stage holds one more row above and below
+// the CTA's rows, and the strip-edge buffer one more slot pair for the rows the partner sends.
+template <int T, int R, int WARPS, int NS, bool CL = false>
 struct Smem {
     static constexpr int TILE_Y = WARPS * R;
-    static constexpr int kStageFloats = TILE_Y * kTileX;
+    static constexpr int kRows = TILE_Y + (CL ? 2 : 0);
+    static constexpr int kSlots = WARPS + (CL ? 1 : 0);
+    static constexpr int kStageFloats = kRows * kTileX;
     static constexpr size_t kStageBytes = (size_t)kStageFloats * sizeof(float);
-    static constexpr size_t kEdgeBytes = (size_t)(T > 1 ? T - 1 : 0) * 2 * WARPS * 2 * kLanes * sizeof(float4);
+    static constexpr size_t kEdgeBytes = (size_t)(T > 1 ? T - 1 : 0) * 2 * kSlots * 2 * kLanes * sizeof(float4);
     static constexpr size_t kBarOff = NS * kStageBytes + kEdgeBytes;
-    static constexpr size_t kBytes = kBarOff + NS * sizeof(uint64_t);
+    static constexpr int kXBars = CL ? 2 : 0;           // CL: one per plane parity for the partner's rows of all levels
+    static constexpr size_t kBytes = kBarOff + (NS + kXBars) * sizeof(uint64_t);
 };
 
 // ONE: the cube has at most 128 columns, so a single tile column covers a row with all 32 lanes valid and no halo
 // lanes; the x faces are replicated by patching the shuffled neighbour of the first / last float4 of the row.
 // UNAL: nx % 4 != 0 -- the buffers are pitched copies (row pitch L.pitch), the x face at nx - 1 lies INSIDE a float4:
 // cells beyond it take the even reflection element by element (cell x <- cell 2 nx - 1 - x) from the level-0 stage.
-template <int TL, int R, int WARPS, int NS, int TMAX, bool ONE, bool PM = false, bool UNAL = false>
+// CL: the CTA is one of a cluster pair stacked along y.  The pair covers 2 TILE_Y rows with the T halo rows at its two
+// OUTER edges only (useful rows 2 TILE_Y - 2 T of 2 TILE_Y, against TILE_Y - 2 T of TILE_Y alone); across the seam the
+// two CTAs exchange the strip-edge rows of every fused level through distributed shared memory: the warp at the seam
+// sends its row with st.async into the partner's edge buffer, completion counted on an mbarrier of the partner, and
+// waits on its own mbarrier for the partner's row -- no cluster-wide barrier in the plane loop (a release at cluster
+// scope would also wait for the global stores of the plane).  A CTA reads the partner's row of the previous plane
+// BEFORE it sends its own of this plane, so the partner, which needs that row to go on, cannot overwrite a slot that
+// is still to be read; the two CTAs stay within one plane of each other.
+template <int TL, int R, int WARPS, int NS, int TMAX, bool ONE, bool PM = false, bool UNAL = false, bool CL = false>
 __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restrict__ dst, const Launch &L,
                                          const TmaArgs &A, const CubeParams &prm, int b,
                                          unsigned char *smem, bool reinit = false)
 {
-    using S = Smem<TMAX, R, WARPS, NS>;
+    using S = Smem<TMAX, R, WARPS, NS, CL>;
     constexpr int TILE_Y = WARPS * R;
+    constexpr int RB = CL ? 1 : 0;                       // stage row of the CTA's row 0
     float *stage0 = reinterpret_cast<float *>(smem);
     float4 *edge = reinterpret_cast<float4 *>(smem + NS * S::kStageBytes);
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + S::kBarOff);
@@ -80,10 +94,12 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
     const int wy = threadIdx.x >> 5;
     const int nx4 = UNAL ? (L.nx + 3) >> 2 : L.nx >> 2;       // float4 columns that hold cube voxels
     const int ld = UNAL ? L.pitch : L.nx;                      // row pitch of the buffers
-    const int vy = TILE_Y - 2 * A.halo;
-    const int ti = blockIdx.x % A.tiles_x, tj = blockIdx.x / A.tiles_x;
+    const int rank = CL ? (int)(blockIdx.x & 1u) : 0;     // position in the cluster pair (0: upper rows)
+    const int tile = CL ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
+    const int vy = (CL ? 2 : 1) * TILE_Y - 2 * A.halo;
+    const int ti = tile % A.tiles_x, tj = tile / A.tiles_x;
     const int tx0 = ONE ? 0 : (ti * kValidLanes - 1) * 4;   // cube x of tile column 0
-    const int ty0 = tj * vy - A.halo;                    // cube y of tile row 0
+    const int ty0 = tj * vy - A.halo + rank * TILE_Y;    // cube y of the CTA's row 0
     const int x4 = ONE ? lane : ti * kValidLanes - 1 + lane;
     const bool x_first = ONE && lane == 0, x_last = ONE && lane == nx4 - 1;
     const int row0 = wy * R;
@@ -107,20 +123,38 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int row = row0 + r, gy = ty0 + row;
-        cell[r] = row * kTileX + lane * 4;
+        cell[r] = (row + RB) * kTileX + lane * 4;
         int srow = row;
         if (gy < 0) srow = (-1 - gy) - ty0;
         else if (gy >= L.ny) srow = (2 * L.ny - 1 - gy) - ty0;
-        if (srow < 0 || srow >= TILE_Y) srow = row;
-        scell[r] = srow * kTileX + slane * 4;
+        if (srow < -RB || srow >= TILE_Y + RB) srow = row;
+        scell[r] = (srow + RB) * kTileX + slane * 4;
         if (scell[r] != cell[r] || xfix) fix |= 1u << r;
-        if ((ONE || (lane >= 1 && lane <= kValidLanes)) && x4 < nx4 && row >= A.halo && row < TILE_Y - A.halo &&
-            gy < L.ny)
+        if ((ONE || (lane >= 1 && lane <= kValidLanes)) && x4 < nx4 && (row >= A.halo || (CL && rank == 1)) &&
+            (row < TILE_Y - A.halo || (CL && rank == 0)) && gy < L.ny)
             ok |= 1u << r;
     }
-    const int up_cell = max(row0 - 1, 0) * kTileX + lane * 4;              // level-0 strip-edge rows
-    const int dn_cell = min(row0 + R, TILE_Y - 1) * kTileX + lane * 4;
-    const int wy_up = max(wy - 1, 0), wy_dn = min(wy + 1, WARPS - 1);
+    // level-0 strip-edge rows (plane q-1 of the stage).  CL: the stage has the rows -1 and TILE_Y too; a neighbour row
+    // beyond the cube's last row is its mirror image, the strip's own last row (the seam may lie on the face)
+    int up_row = CL ? row0 - 1 : max(row0 - 1, 0), dn_row = CL ? row0 + R : min(row0 + R, TILE_Y - 1);
+    if (CL && ty0 + dn_row >= L.ny && ty0 + dn_row - 1 >= 0) dn_row = min(max(2 * L.ny - 1 - (ty0 + dn_row) - ty0, -1), TILE_Y);
+    if (CL && ty0 + up_row < 0) up_row = min(max(-1 - (ty0 + up_row) - ty0, -1), TILE_Y);
+    // (CL: rows -1 and TILE_Y of a stage have no owner that would write the x-reflected cells back: read the source lane)
+    const int up_cell = (up_row + RB) * kTileX + (CL ? slane : lane) * 4;
+    const int dn_cell = (dn_row + RB) * kTileX + (CL ? slane : lane) * 4;
+    // slots of the strip-edge buffer my up / down neighbour rows come from; CL: slot WARPS holds what the partner sent
+    const int wy_up = (CL && rank == 1 && wy == 0) ? WARPS : max(wy - 1, 0);
+    const int wy_dn = (CL && rank == 0 && wy == WARPS - 1) ? WARPS : min(wy + 1, WARPS - 1);
+    // CL: the warp at the seam also writes its seam row into the partner's slot WARPS (the row the partner lacks)
+    const bool seam = CL && ((rank == 0 && wy == WARPS - 1) || (rank == 1 && wy == 0));
+    uint32_t peer_edge = 0, peer_xbar = 0;
+    const uint32_t xbar = ptx::smem_u32(smem + S::kBarOff + NS * sizeof(uint64_t));
+    if (CL) {
+        const uint32_t mine = ptx::smem_u32(smem + NS * S::kStageBytes);
+        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(peer_edge) : "r"(mine), "r"(rank ^ 1));
+        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(peer_xbar) : "r"(xbar), "r"(rank ^ 1));
+    }
+    const uint32_t send_base = peer_edge + (uint32_t)((WARPS * 2 + (rank == 0 ? 1 : 0)) * kLanes + lane) * 16u;
 
     const size_t plane = (size_t)ld * (size_t)L.ny;
     float *po = dst + (long long)(ty0 + row0) * ld + (long long)x4 * 4 + (long long)(q_first - TL - 1) * (long long)plane;
@@ -131,13 +165,22 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
             if (reinit) ptx::mbar_inval(ptx::smem_u32(&full[s]));      // a later round of a cooperative launch
             mbar_init(&full[s], 1);
         }
+        if (CL) {
+#pragma unroll
+            for (int i = 0; i < S::kXBars; ++i) ptx::mbar_init(xbar + 8 * i, 1);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    __syncthreads();
+    if (CL) {                   // the partner runs: its shared memory may be written from here on
+        ptx::cluster_arrive();
+        ptx::cluster_wait();
+    } else {
+        __syncthreads();
+    }
     auto issue = [&](int q) {       // thread 0: plane q -> stage (q - q_first) % NS
         const int s = (q - q_first) % NS;
         mbar_expect_tx(&full[s], (uint32_t)S::kStageBytes);
-        tma_load_4d(stage0 + (size_t)s * S::kStageFloats, map, &full[s], tx0, ty0, mirror(q, L.nz), b);
+        tma_load_4d(stage0 + (size_t)s * S::kStageFloats, map, &full[s], tx0, ty0 - RB, mirror(q, L.nz), b);
     };
     if (threadIdx.x == 0) {
 #pragma unroll
@@ -170,6 +213,14 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             issue(q + NS - 2);                              // its stage held plane q-2: free since last barrier
         }
+        // CL: the partner's seam rows of the previous plane (every level) are normally in by now: ask early, so that
+        // the answer is there when level 1 needs the rows
+        bool xready = true;
+        if (CL && TL > 1 && seam && it > 0) {
+            const uint32_t mb = xbar + 8u * (uint32_t)par;
+            if (lane == 0) ptx::mbar_expect_tx(mb, (uint32_t)(TL - 1) * kLanes * 16u);
+            xready = ptx::mbar_test(mb, ((it - 1u) >> 1) & 1u);
+        }
         const float *st = stage0 + (size_t)s * S::kStageFloats;                      // plane q
         const float *stp = stage0 + (size_t)((it + NS - 1) % NS) * S::kStageFloats;  // plane q-1
         mbar_wait(&full[s], (uint32_t)((it / NS) & 1));
@@ -201,16 +252,29 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
             if (t == 0) {
                 up = lds4(stp + up_cell);
                 dn = lds4(stp + dn_cell);
+                if (CL && rev) {
+                    up = F4{up.w, up.z, up.y, up.x};
+                    dn = F4{dn.w, dn.z, dn.y, dn.x};
+                }
             } else {
-                float4 *e_rd = edge + (((t - 1) * 2 + par) * WARPS) * 2 * kLanes;
-                float4 *e_wr = edge + (((t - 1) * 2 + (par ^ 1)) * WARPS) * 2 * kLanes;
+                float4 *e_rd = edge + (((t - 1) * 2 + par) * S::kSlots) * 2 * kLanes;
+                float4 *e_wr = edge + (((t - 1) * 2 + (par ^ 1)) * S::kSlots) * 2 * kLanes;
                 e_wr[(wy * 2 + 0) * kLanes + lane] = make_float4(nw[t][0].x, nw[t][0].y, nw[t][0].z, nw[t][0].w);
                 e_wr[(wy * 2 + 1) * kLanes + lane] =
                     make_float4(nw[t][R - 1].x, nw[t][R - 1].y, nw[t][R - 1].z, nw[t][R - 1].w);
+                if (CL && t == 1 && !xready) ptx::mbar_wait_spin(xbar + 8u * (uint32_t)par, ((it - 1u) >> 1) & 1u);
                 const float4 u = e_rd[(wy_up * 2 + 1) * kLanes + lane];
                 const float4 d = e_rd[(wy_dn * 2 + 0) * kLanes + lane];
                 up = F4{u.x, u.y, u.z, u.w};
                 dn = F4{d.x, d.y, d.z, d.w};
+                if (CL && seam) {               // only now my seam row of this plane -> the partner's slot WARPS
+                    // (the loaded neighbour row is an operand: the send cannot be scheduled ahead of that load)
+                    const F4 &v = rank == 0 ? nw[t][R - 1] : nw[t][0];
+                    const uint32_t a = send_base + (uint32_t)((t - 1) * 2 + (par ^ 1)) * (uint32_t)(S::kSlots * 2 * kLanes * 16);
+                    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1, %2, %3, %4}, [%5];"
+                                 ::"r"(a), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "r"(peer_xbar + 8u * (uint32_t)(par ^ 1)),
+                                   "f"(rank == 0 ? d.x : u.x));
+                }
             }
 #pragma unroll
             for (int r = 0; r < R; ++r) {
@@ -251,9 +315,13 @@ __device__ __forceinline__ void tma_body(const CUtensorMap *map, float *__restri
         step(std::integral_constant<int, 2>{});
         if (q > q_last) break;
     }
+    if (CL) {                           // neither CTA leaves while the other may still send into its shared memory
+        ptx::cluster_arrive();
+        ptx::cluster_wait();
+    }
 }
 
-template <int T, int R, int WARPS, int NS, int MINB, bool ONE, bool PM = false, bool UNAL = false>
+template <int T, int R, int WARPS, int NS, int MINB, bool ONE, bool PM = false, bool UNAL = false, bool CL = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 idg_tma_kernel(const __grid_constant__ Launch L, const __grid_constant__ TmaArgs A,
                const __grid_constant__ Maps M)
@@ -264,13 +332,13 @@ idg_tma_kernel(const __grid_constant__ Launch L, const __grid_constant__ TmaArgs
     const float *src;
     float *dst;
     const int now = route(L, b, prm, src, dst);
-    if (now == 0) return;
+    if (now == 0) return;               // (both CTAs of a cluster pair: same cube)
     const size_t off = (size_t)b * cube_stride(L);
     const CUtensorMap *map = (src == L.scratch + off) ? &M.scratch : (src == L.out + off) ? &M.out : &M.in;
-    if (now == T) tma_body<T, R, WARPS, NS, T, ONE, PM, UNAL>(map, dst, L, A, prm, b, smem);
-    else if (T > 1 && now == 1) tma_body<1, R, WARPS, NS, T, ONE, PM, UNAL>(map, dst, L, A, prm, b, smem);
-    else if (T > 2 && now == 2) tma_body<(T > 2 ? 2 : 1), R, WARPS, NS, T, ONE, PM, UNAL>(map, dst, L, A, prm, b, smem);
-    else if (T > 3 && now == 3) tma_body<(T > 3 ? 3 : 1), R, WARPS, NS, T, ONE, PM, UNAL>(map, dst, L, A, prm, b, smem);
+    if (now == T) tma_body<T, R, WARPS, NS, T, ONE, PM, UNAL, CL>(map, dst, L, A, prm, b, smem);
+    else if (T > 1 && now == 1) tma_body<1, R, WARPS, NS, T, ONE, PM, UNAL, CL>(map, dst, L, A, prm, b, smem);
+    else if (T > 2 && now == 2) tma_body<(T > 2 ? 2 : 1), R, WARPS, NS, T, ONE, PM, UNAL, CL>(map, dst, L, A, prm, b, smem);
+    else if (T > 3 && now == 3) tma_body<(T > 3 ? 3 : 1), R, WARPS, NS, T, ONE, PM, UNAL, CL>(map, dst, L, A, prm, b, smem);
 }
 
 // Cooperative variant: all `A.rounds` launches of a plan in one, a grid barrier between rounds (the whole grid is
@@ -330,14 +398,26 @@ int pick_zchunk(int nz, long tiles, int T, int slots, long max_ctas = 0)
     return best;
 }
 
+// The cluster-pair tiling is valid unless the cube's last row lies within a few rows of a seam between the two CTAs of a
+// pair: rows beyond a face take their mirror images from the CTA's own stage, and those would be the partner's rows.
+bool pair_tiling_ok(int ny, int tile_y, int T)
+{
+    const int vy = 2 * tile_y - 2 * T;
+    const int last = (ny + vy - 1) / vy - 1;
+    const int f = ny - (last * vy - T + tile_y);         // rows of the last pair's lower CTA that lie inside the cube
+    return f < -(T - 1) || f > T - 2;
+}
+
 // rounds > 1: cooperative launch of all rounds (COOP instantiation); the grid must be co-resident.
-template <int T, int R, int WARPS, int NS, int MINB, bool COOP = false, bool PM = false>
+// pair: two CTAs of a cluster share a tile of 2 TILE_Y rows (T >= 2, plain launches, aligned rows only).
+template <int T, int R, int WARPS, int NS, int MINB, bool COOP = false, bool PM = false, bool PAIR = false>
 cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st, int rounds = 1, unsigned *bar = nullptr)
 {
-    using S = Smem<T, R, WARPS, NS>;
+    using S = Smem<T, R, WARPS, NS, PAIR>;
     constexpr int TILE_Y = WARPS * R;
     static_assert(TILE_Y > 2 * T, "tile must be taller than its halo");
     static_assert(S::kBytes * MINB <= 227 * 1024, "shared memory budget");
+    static_assert(!(PAIR && (COOP || PM)), "the cluster-pair tiling exists for the plain intensity-driven kernel");
     constexpr bool coop = COOP;
     TmaArgs A;
     A.halo = T;
@@ -345,18 +425,21 @@ cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st, int rounds 
     A.bar = bar;
     const bool unal = L.pitch > 0;                       // nx % 4 != 0: pitched buffers, the face inside a float4
     const bool one = L.nx <= kTileX && !unal;            // a single tile column: no halo lanes
+    if (PAIR && (unal || one)) return cudaErrorNotSupported;
     A.tiles_x = one ? 1 : ((L.nx + 3) / 4 + kValidLanes - 1) / kValidLanes;
-    A.tiles_y = (L.ny + (TILE_Y - 2 * T) - 1) / (TILE_Y - 2 * T);
-    const long tiles = (long)A.tiles_x * A.tiles_y;
+    const int vy = (PAIR ? 2 : 1) * TILE_Y - 2 * T;
+    A.tiles_y = (L.ny + vy - 1) / vy;
+    const long tiles = (long)A.tiles_x * A.tiles_y * (PAIR ? 2 : 1);        // CTAs per cube and z chunk
     if (tiles > 0x7fffffffL) return cudaErrorInvalidValue;
     void (*kern)(Launch, TmaArgs, Maps);
     if constexpr (COOP) kern = one ? idg_tma_coop_kernel<T, R, WARPS, NS, MINB, true> : idg_tma_coop_kernel<T, R, WARPS, NS, MINB, false>;
+    else if constexpr (PAIR) kern = idg_tma_kernel<T, R, WARPS, NS, MINB, false, false, false, true>;
     else if (unal && !PM) kern = idg_tma_kernel<T, R, WARPS, NS, MINB, false, false, !PM>;      // (!PM: no pm instantiation)
     else kern = one ? idg_tma_kernel<T, R, WARPS, NS, MINB, true, PM> : idg_tma_kernel<T, R, WARPS, NS, MINB, false, PM>;
     if (unal && (COOP || PM)) return cudaErrorNotSupported;
-    static DeviceOnce smem_once[3];
+    static DeviceOnce smem_once[4];
     {
-        const cudaError_t e = set_max_dynamic_smem(smem_once[unal ? 2 : one], (const void *)kern, S::kBytes);
+        const cudaError_t e = set_max_dynamic_smem(smem_once[PAIR ? 3 : unal ? 2 : one], (const void *)kern, S::kBytes);
         if (e != cudaSuccess) return e;
     }
     const int sms = device_sm_count();
@@ -374,14 +457,29 @@ cudaError_t launch_cfg(const Launch &L, int zchunk, cudaStream_t st, int rounds 
     }
     if ((L.nz + A.zchunk - 1) / A.zchunk > 65535) A.zchunk = (L.nz + 65534) / 65535;
     Maps M;
-    if (!encode_map(&M.in, L.in, L, TILE_Y) || !encode_map(&M.out, L.out, L, TILE_Y) ||
-        !encode_map(&M.scratch, L.scratch, L, TILE_Y))
+    if (!encode_map(&M.in, L.in, L, S::kRows) || !encode_map(&M.out, L.out, L, S::kRows) ||
+        !encode_map(&M.scratch, L.scratch, L, S::kRows))
         return cudaErrorNotSupported;
     dim3 grid((unsigned)tiles, (unsigned)((L.nz + A.zchunk - 1) / A.zchunk), (unsigned)L.batch);
     if (coop) {
         if ((long)grid.x * grid.y * grid.z > slots) return cudaErrorCooperativeLaunchTooLarge;
         void *args[3] = {(void *)&L, (void *)&A, (void *)&M};
         return cudaLaunchCooperativeKernel((const void *)kern, grid, dim3(WARPS * 32), args, S::kBytes, st);
+    }
+    if constexpr (PAIR) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = grid;
+        cfg.blockDim = dim3(WARPS * 32);
+        cfg.dynamicSmemBytes = S::kBytes;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        return cudaLaunchKernelEx(&cfg, kern, L, A, M);
     }
     kern<<<grid, WARPS * 32, S::kBytes, st>>>(L, A, M);
     return cudaGetLastError();
@@ -456,11 +554,19 @@ cudaError_t launch_tma(const Launch &L, int zchunk, int tile, cudaStream_t st)
     case 3:
         switch (tile) {
         case 3: return launch_cfg<3, 4, 12, 4, 1>(L, zchunk, st);
+        case 4:
+            if (L.nx > kTileX && L.pitch == 0 && pair_tiling_ok(L.ny, 32, 3))
+                return launch_cfg<3, 4, 8, 4, 1, false, false, true>(L, zchunk, st);
+            return launch_cfg<3, 4, 8, 4, 1>(L, zchunk, st);
         default: return launch_cfg<3, 4, 8, 4, 1>(L, zchunk, st);
         }
     case 4:
         switch (tile) {
         case 3: return launch_cfg<4, 3, 12, 4, 1>(L, zchunk, st);
+        case 4:
+            if (L.nx > kTileX && L.pitch == 0 && pair_tiling_ok(L.ny, 32, 4))
+                return launch_cfg<4, 4, 8, 4, 1, false, false, true>(L, zchunk, st);
+            return launch_cfg<4, 4, 8, 4, 1>(L, zchunk, st);
         default: return launch_cfg<4, 4, 8, 4, 1>(L, zchunk, st);
         }
     default: return cudaErrorInvalidValue;

@@ -97,11 +97,12 @@ def test_zchunk_variants(B, oracle, kernel, fuse, zchunk):
     assert err(gpu(B, a, 7, p), ref, 2.0) <= TOL
 
 
-@pytest.mark.parametrize("tile", [1, 2, 3])
+@pytest.mark.parametrize("tile", [1, 2, 3, 4])
 @pytest.mark.parametrize("fuse", [1, 2, 3, 4])
 def test_tma_tile_variants(B, oracle, fuse, tile):
     """The tilings of the TMA kernel (T <= 2: 128x64 one CTA/SM, 128x32 two CTAs/SM; T >= 3: 8 or 12 warps
-    of one CTA/SM) on a cube spanning several tiles in x and y with ragged tails, and on the config-0
+    of one CTA/SM, or -- tile 4 -- cluster pairs of two CTAs stacked along y that exchange their seam rows through
+    distributed shared memory) on a cube spanning several tiles in x and y with ragged tails, and on the config-0
     cube; n = 6 and 10 also exercise the tail launch of n mod T iterations."""
     from paper_1609_03782_b200 import synth
     set_plan(B, (3, fuse), 0, tile)
@@ -577,6 +578,24 @@ def test_unaligned_rows_run_the_tma_kernel_on_pitched_copies(B, oracle, nx):
     assert err(ref1.cpu().numpy(), want, 1.0) <= TOL
 
 
+@pytest.mark.parametrize("ny", [24, 25, 31, 52, 55, 56, 57, 60, 84, 87, 88, 111, 112, 113, 140, 300])
+def test_cluster_pair_tiling_is_bitwise_equal_to_the_naive_kernel(B, ny):
+    """IDG_OPT_TILE = 4 (T = 3, 4): two CTAs of a cluster share a 128 x 64 tile with the T halo rows at its outer edges
+    only; the strip-edge rows of every fused level cross the seam by st.async + mbarrier.  Any position of the cube's
+    last row relative to a seam (the host falls back to single-CTA tiles where the mirror rows would be the partner's),
+    several runs each: a row read before it arrived would show as a differing voxel."""
+    g = torch.Generator(device="cuda").manual_seed(ny)
+    x = torch.randn((13, ny, 268), device="cuda", generator=g) * 2.0
+    p = B.Params(K=1.5, tau=0.03, cx=5.0, cy=4.0, cz=6.0, rms=1.0)
+    set_plan(B, (1, 0))
+    ref = B.idg_filter(x, 9, p)
+    for fuse in (3, 4):
+        for rep in range(3):
+            set_plan(B, (3, fuse), 0, 4)
+            out = B.idg_filter(x, 9, p)
+            assert torch.equal(out, ref), (ny, fuse, rep, int((out != ref).sum()))
+
+
 @pytest.mark.parametrize("plan", [(2, 2), (3, 1), (3, 2), (3, 3), (3, 4)],
                          ids=lambda p: f"k{p[0]}-T{p[1]}")
 def test_fused_kernels_are_bitwise_equal_to_the_naive_kernel_and_repeatable(B, plan):
@@ -589,7 +608,7 @@ def test_fused_kernels_are_bitwise_equal_to_the_naive_kernel_and_repeatable(B, p
     p = B.Params(K=1.5, tau=0.03, cx=5.0, cy=4.0, cz=6.0, rms=1.0)
     set_plan(B, (1, 0))
     ref = B.idg_filter(x, 7, p)
-    for tile in ((1, 2) if plan[0] == 3 and plan[1] <= 2 else ((0, 3) if plan[0] == 3 else (0,))):
+    for tile in ((1, 2) if plan[0] == 3 and plan[1] <= 2 else ((0, 3, 4) if plan[0] == 3 else (0,))):
         for rep in range(4):
             set_plan(B, plan, 0, tile)
             out = B.idg_filter(x, 7, p)
