@@ -505,19 +505,38 @@ bool tma_pitched_supported(int nx, int ny, int nz)
 }
 
 namespace {
-// Row-by-row copy between a dense cube (pitch nx) and its pitched copy; cubes whose n_iter is 0 take src_zero
-// (their untouched input copy) instead of src.
-__global__ void idg_repitch_kernel(const float *__restrict__ src, int src_pitch, float *__restrict__ dst, int dst_pitch,
+// Copy between a dense cube (row pitch nx, rows not 16-byte aligned) and its pitched copy (row pitch a multiple of 4
+// floats): a thread moves one float4 of the pitched side and the 1..4 voxels of it that exist, the dense side by scalar
+// accesses (coalesced across the warp).  TO_PITCHED: dense -> pitched, else pitched -> dense; cubes whose n_iter is 0
+// take src_zero (their untouched input copy) instead of src.
+template <bool TO_PITCHED>
+__global__ void idg_repitch_kernel(const float *__restrict__ src, float *__restrict__ dst, int pitch,
                                    const float *__restrict__ src_zero, const CubeParams *__restrict__ tab, int nx,
                                    size_t rows_per_cube, size_t rows)
 {
-    for (size_t row = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); row < rows;
-         row += (size_t)gridDim.x * (blockDim.x >> 5)) {
-        const float *s = src;
-        if (src_zero && tab && tab[row / rows_per_cube].n_iter == 0) s = src_zero;
-        const float *sr = s + row * (size_t)src_pitch;
-        float *dr = dst + row * (size_t)dst_pitch;
-        for (int x = threadIdx.x & 31; x < nx; x += 32) dr[x] = sr[x];
+    const int p4 = pitch >> 2;
+    const size_t total = rows * (size_t)p4;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t row = i / (size_t)p4;
+        const int x = (int)(i - row * (size_t)p4) * 4;
+        if (TO_PITCHED) {
+            const float *sr = src + row * (size_t)nx + x;
+            float4 v;
+            v.x = sr[0];
+            v.y = x + 1 < nx ? sr[1] : 0.f;
+            v.z = x + 2 < nx ? sr[2] : 0.f;
+            v.w = x + 3 < nx ? sr[3] : 0.f;
+            *reinterpret_cast<float4 *>(dst + row * (size_t)pitch + x) = v;
+        } else {
+            const float *s = src;
+            if (src_zero && tab && tab[row / rows_per_cube].n_iter == 0) s = src_zero;
+            const float4 v = *reinterpret_cast<const float4 *>(s + row * (size_t)pitch + x);
+            float *dr = dst + row * (size_t)nx + x;
+            dr[0] = v.x;
+            if (x + 1 < nx) dr[1] = v.y;
+            if (x + 2 < nx) dr[2] = v.z;
+            if (x + 3 < nx) dr[3] = v.w;
+        }
     }
 }
 }  // namespace
@@ -526,10 +545,14 @@ cudaError_t launch_repitch(const float *src, int src_pitch, float *dst, int dst_
                            const CubeParams *tab, int nx, int ny, int nz, int batch, cudaStream_t st)
 {
     const size_t rows_per_cube = (size_t)ny * (size_t)nz, rows = rows_per_cube * (size_t)batch;
-    size_t blocks = (rows + 7) / 8;
-    const size_t cap = (size_t)device_sm_count() * 32;
+    const bool to_pitched = dst_pitch > src_pitch;
+    const int pitch = to_pitched ? dst_pitch : src_pitch;
+    const size_t total = rows * (size_t)(pitch / 4);
+    size_t blocks = (total + 255) / 256;
+    const size_t cap = (size_t)device_sm_count() * 16;
     if (blocks > cap) blocks = cap;
-    idg_repitch_kernel<<<(unsigned)blocks, 256, 0, st>>>(src, src_pitch, dst, dst_pitch, src_zero, tab, nx, rows_per_cube, rows);
+    if (to_pitched) idg_repitch_kernel<true><<<(unsigned)blocks, 256, 0, st>>>(src, dst, pitch, nullptr, nullptr, nx, rows_per_cube, rows);
+    else idg_repitch_kernel<false><<<(unsigned)blocks, 256, 0, st>>>(src, dst, pitch, src_zero, tab, nx, rows_per_cube, rows);
     return cudaGetLastError();
 }
 
