@@ -44,7 +44,7 @@ struct ResArgs {
     int ty, tz;                     // blocks per cube along y, z
     int by, bz;                     // nominal block extents (the last block of an axis may be smaller)
     int ls;                         // z cells per work item
-    int words;                      // 64-bit words per (block, parity): 2 nx (by + bz)
+    int words;                      // 64-bit words per (block, parity): 2 nx (by + bz) of faces + 8 (4 flags)
     unsigned m_nx4;                 // ceil(2^32 / (nx / 4)): division by multiplication
 };
 
@@ -329,8 +329,28 @@ __global__ void __launch_bounds__(kThreads, 1) idg_resident_kernel(const __grid_
             const unsigned tag = (unsigned)it;
             const int pw = (it & 1) * A.words;
             for (int wi = warp; wi < nwitems; wi += kThreads / 32) run_item(decode(wi), xchg, tag, pw);
-            if (xchg) {          // my neighbours' faces of this iterate -> the frame of `nxt`
-                for (int e = tid; e < n_in; e += kThreads) {
+            if (xchg) {
+                // Large blocks: polling every face entry from the moment the block is computed floods the L2 with
+                // requests (12 rounds per entry were measured) that delay the very stores they wait for.  So a CTA
+                // raises one flag per face AFTER all its warps have issued their face stores, the receiver waits on
+                // its four flags with four threads, and only then reads the faces -- once, as a rule; every entry
+                // still carries its tag and is re-read until it matches (flag and data are not ordered).
+                __syncthreads();
+                const int fl = A.words - 8;
+                if (tid < 4) {
+                    const int nb = tid == 0 ? nb_ym : tid == 1 ? nb_yp : tid == 2 ? nb_zm : nb_zp;
+                    if (nb >= 0) {
+                        unsigned long long *f = A.mail + (size_t)nb * 2 * A.words + pw + fl + (tid ^ 1);
+                        asm volatile("st.relaxed.gpu.global.b64 [%0], %1;" ::"l"(f), "l"((unsigned long long)tag));
+                        const unsigned long long *mine = inbox + pw + fl + tid;
+                        unsigned long long v;
+                        do {
+                            asm volatile("ld.relaxed.gpu.global.b64 %0, [%1];" : "=l"(v) : "l"(mine));
+                        } while (v != (unsigned long long)tag);
+                    }
+                }
+                __syncthreads();
+                for (int e = tid; e < n_in; e += kThreads) {     // my neighbours' faces of this iterate -> the frame of `nxt`
                     const Inbound in = inbound(e);
                     if (in.lo) sts4(nxt + in.dst, pull(in.lo + pw, in.hi, tag));
                 }
@@ -417,7 +437,7 @@ bool search_plan(int nx, int ny, int nz, int batch, int max_n, size_t mail_bytes
             if (smem > kSmemBudget) continue;
             const int per_wave = sms / (ty * tz);                   // cubes per launch
             const int cubes = per_wave < batch ? per_wave : batch;
-            const size_t words = (size_t)2 * nx * (by + bz);
+            const size_t words = (size_t)2 * nx * (by + bz) + 8;      // faces + one arrival flag per face
             if ((size_t)cubes * ty * tz * 2 * words * 8 > mail_bytes) continue;
             const int waves = (batch + per_wave - 1) / per_wave;
             // a warp item = 32 columns x ls cells; pick the segment length that balances the 16 warps best
