@@ -426,10 +426,18 @@ def run_ours(args) -> None:
         return
 
     peak, peak_src = measured_peak_gbs()
-    ms_launch = ms_step / launches_per_step
+    roof_launches = launches_per_step
     if filt is not None and filt[0] == "wavelet":      # many small passes: the roofline unit is the whole filter
-        ms_launch, fuse = ms_step, 1
-    alg_bytes = BYTES_PER_VOXEL_ITER * voxel_iters / launches_per_step        # algorithmic bytes per launch
+        roof_launches, fuse = 1, 1
+    ms_launch = ms_step / roof_launches
+    alg_bytes = BYTES_PER_VOXEL_ITER * voxel_iters / roof_launches            # algorithmic bytes per launch
+    if filt is None and "fuse=" in plan:               # iterations the dominant kernel fuses (a sweep mixes tails in)
+        try:
+            fuse = max(fuse, int(plan.split("fuse=")[1].split()[0]))
+        except ValueError:
+            pass
+    if "idg_resident" in plan:
+        fuse = n
     hbm_equiv = alg_bytes / (ms_launch * 1e-3) / 1e9
     ncu = ncu_counters(plan, args.workload)
     traffic = ncu.get("dram_bytes")
@@ -478,14 +486,17 @@ def run_ours(args) -> None:
     roof = {"bound": "hbm", "achieved": hbm_equiv, "peak": peak, "unit": "GB/s", "frac": hbm_equiv / peak,
             "traffic": traffic, "kernel": plan, "ms_per_launch": ms_launch,
             "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src}
-    if fused_idg:
-        wi = ncu.get("warp_instructions")
+    wi = ncu.get("warp_instructions")
+    if fused_idg and wi:
         roof.update({"bound": "alu", "unit": "T warp-inst/s", "peak": issue_peak,
                      "achieved": (wi / (ms_launch * 1e-3) / 1e12) if wi else None,
                      "frac": (wi / (ms_launch * 1e-3) / 1e12 / issue_peak) if wi else None,
                      "peak_source": "derived: 148 SMs x 4 warp schedulers x 1.965 GHz (B200_PROFILING.md)",
                      "warp_instructions_per_launch": wi,
-                     "useful_thread_inst_per_voxel_iter": (wi * 32 / (voxel_iters / launches_per_step)) if wi else None})
+                     "useful_thread_inst_per_voxel_iter": (wi * 32 / (voxel_iters / roof_launches)) if wi else None})
+    elif fused_idg:
+        roof["note_bound"] = ("a fused IDG plan is bound by instruction issue, not HBM; no ncu instruction count of this plan on "
+                              "this workload is committed, so only the HBM-equivalent figure is given")
     roof["hbm_equiv_gbs"] = hbm_equiv
     roof["hbm_equiv_frac"] = hbm_equiv / peak
     roof["hbm_peak_gbs"] = peak
@@ -496,7 +507,7 @@ def run_ours(args) -> None:
         l2b = ncu.get("l2_bytes")
         roof["l2"] = {"bytes_per_launch": l2b, "gbs": (l2b / (ms_launch * 1e-3) / 1e9) if l2b else None,
                       "peak_gbs": L2_PEAK_GBS, "frac": (l2b / (ms_launch * 1e-3) / 1e9 / L2_PEAK_GBS) if l2b else None,
-                      "note": "lts__t_bytes.sum of the ncu capture over the launch time measured here"}
+                      "note": "L2 -> SM read bytes (l1tex__m_xbar2l1tex_read_bytes.sum) of the ncu capture over the launch time measured here"}
     roof["note"] = ("algorithmic bytes = 8 B x voxel-iterations of a launch (what an un-fused sweep must move); temporal "
                     "fusion moves fewer DRAM bytes, so hbm_equiv_frac can exceed 1 -- dram_frac_actual is the real HBM load")
     line = {
