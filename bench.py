@@ -77,10 +77,10 @@ def measured_peak_gbs():
 
 def ncu_counters(plan: str, workload: str) -> dict:
     """Per-launch ncu counters of the dominant kernel of (plan, workload) from the committed table
-    profiles/ncu_per_launch.json (each entry names its source note and commit); {} when this plan on this workload
+    profiles/ncu_per_launch.txt (each entry names its source note and commit); {} when this plan on this workload
     has never been captured -- then the line carries no traffic figure rather than someone else's."""
     try:
-        with open(os.path.join(ROOT, "profiles", "ncu_per_launch.json")) as f:
+        with open(os.path.join(ROOT, "profiles", "ncu_per_launch.txt")) as f:
             for e in json.load(f)["entries"]:
                 if e["plan"] == plan and e["workload"] == workload:
                     return e
@@ -478,7 +478,7 @@ def run_ours(args) -> None:
 
     # Which ceiling binds.  The temporally fused IDG kernels are bound by FP32 issue, not by HBM:
     # the roof is the SMs' instruction issue rate (148 SMs x 4 schedulers x 1.965 GHz, B200_PROFILING.md unit counts)
-    # and `achieved` is the MEASURED warp-instruction count of this plan (ncu, profiles/ncu_per_launch.json) over the
+    # and `achieved` is the MEASURED warp-instruction count of this plan (ncu, profiles/ncu_per_launch.txt) over the
     # launch time measured live here.  hbm_equiv_frac keeps north_star's figure (8 B per voxel-iteration over the
     # copy bandwidth: > 1 means the fusion beats an un-fused sweep); dram_frac_actual is what really crosses the HBM pins.
     issue_peak = 148 * 4 * 1.965e9 / 1e12              # T warp-instructions / s

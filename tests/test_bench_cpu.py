@@ -71,7 +71,7 @@ def test_reference_arm_under_torchrun_world2():
 
 
 def test_ncu_counter_table_lookup():
-    """bench.py's `roofline.traffic`, its ALU figures and L2 bytes come from profiles/ncu_per_launch.json, keyed by
+    """bench.py's `roofline.traffic`, its ALU figures and L2 bytes come from profiles/ncu_per_launch.txt, keyed by
     (plan, workload); every entry names the note and commit it was measured at, and a plan that was never captured
     on a workload gets nothing (the line then withholds the figures instead of borrowing another plan's)."""
     sys.path.insert(0, ROOT)
@@ -80,7 +80,7 @@ def test_ncu_counter_table_lookup():
     assert 4.2e9 < e["dram_bytes"] < 4.6e9 and e["warp_instructions"] > 9e8 and "source" in e and "commit" in e
     assert bench.ncu_counters("no such kernel", "cfg3_1024x1024x512_n20") == {}
     assert bench.ncu_counters("idg_tma_kernel fuse=4 tile=0", "cfg0_100x100x67_n10") == {}
-    table = json.load(open(os.path.join(ROOT, "profiles", "ncu_per_launch.json")))["entries"]
+    table = json.load(open(os.path.join(ROOT, "profiles", "ncu_per_launch.txt")))["entries"]
     for entry in table:
         assert os.path.exists(os.path.join(ROOT, entry["source"].split(" ")[0])), entry["source"]
         assert entry["workload"] in bench.WORKLOADS
