@@ -46,6 +46,7 @@ L2_PEAK_GBS = 6300 * 1.965          # ~6300 B/clk chip-wide LTS cap x 1.965 GHz 
 # reference filters (PAPER.md:402-405 timing parameters); --filter idg is the contract's metric
 FILTERS = {"idg": None, "box": ("box", (3, 3, 3)), "box_aniso": ("box", (3, 5, 5)),
            "gauss": ("gauss", (3.0, 3.0, 3.0), (0.0, 0.0, 0.0)), "gauss_aniso": ("gauss", (2.0, 3.0, 3.0), (0.0, 0.0, 0.0)),
+           "gauss5": ("gauss", (5.0, 5.0, 5.0), (0.0, 0.0, 0.0)), "gauss7": ("gauss", (7.0, 7.0, 7.0), (0.0, 0.0, 0.0)),
            "gauss_rot": ("gauss", (2.0, 3.0, 3.0), (10.0, 20.0, 30.0)),
            "mask_sums": ("quality",),
            "wavelet_haar": ("wavelet", 0, (0.5, 0.8, 1.1)), "wavelet_legall": ("wavelet", 1, (1.0, 1.4, 1.7))}   # PAPER.md:222                 # Eq. 13-14 over the whole cube: reads 2 cubes

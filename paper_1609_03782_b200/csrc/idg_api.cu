@@ -534,6 +534,14 @@ static cudaError_t run_sep3d(const float *cube, float *out, int nx, int ny, int 
             return e;
         }
     }
+    if (g_opt[IDG_OPT_KERNEL] != 1 && idg::sep3d_big_supported(nx, ny, nz, r[0], r[1], r[2], cube, out)) {
+        const cudaError_t e = idg::launch_sep3d_big(cube, out, nx, ny, nz, r[0], r[1], r[2], wx, wy, wz,
+                                                    g_opt[IDG_OPT_ZCHUNK], g_opt[IDG_OPT_TILE], st);
+        if (e != cudaErrorNotSupported) {
+            *name = "idg_sep3d_big_kernel";
+            return e;
+        }
+    }
     return idg::launch_sep3d(cube, out, nx, ny, nz, r[0], r[1], r[2], wx, wy, wz, st);
 }
 

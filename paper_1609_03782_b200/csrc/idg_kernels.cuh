@@ -170,6 +170,10 @@ cudaError_t launch_sep3d(const float *in, float *out, int nx, int ny, int nz, in
 bool sep3d_tma_supported(int nx, int ny, int nz, int rx, int ry, int rz, const void *in, const void *out);
 cudaError_t launch_sep3d_tma(const float *in, float *out, int nx, int ny, int nz, int rx, int ry, int rz,
                              const float *wx, const float *wy, const float *wz, int zchunk, int variant, cudaStream_t st);
+// the same for radii 5 .. 9 (idg_sep3d_big.cu): HL halo lanes per side, z window shifted in super-steps
+bool sep3d_big_supported(int nx, int ny, int nz, int rx, int ry, int rz, const void *in, const void *out);
+cudaError_t launch_sep3d_big(const float *in, float *out, int nx, int ny, int nz, int rx, int ry, int rz,
+                             const float *wx, const float *wy, const float *wz, int zchunk, int variant, cudaStream_t st);
 // kern [device]: (2r+1)^3 weights, x fastest
 cudaError_t launch_conv3d(const float *in, float *out, int nx, int ny, int nz, int r, const float *kern,
                           cudaStream_t st);

@@ -37,7 +37,7 @@ SHAPES = [(1, 1, 1), (5, 7, 9), (3, 20, 70), (21, 67, 100), (40, 50, 130), (70, 
 IDS = lambda s: "x".join(map(str, s[::-1])) if isinstance(s, tuple) and len(s) == 3 else None
 
 
-@pytest.mark.parametrize("w", [(1, 1, 1), (3, 3, 3), (3, 5, 5), (9, 9, 9), (33, 1, 7), (5, 33, 1)], ids=str)
+@pytest.mark.parametrize("w", [(1, 1, 1), (3, 3, 3), (3, 5, 5), (9, 9, 9), (33, 1, 7), (5, 33, 1), (13, 19, 11), (11, 3, 19)], ids=str)
 @pytest.mark.parametrize("shape", SHAPES, ids=IDS)
 def test_box(B, oracle, shape, w):
     """Paper widths N_j = 1..9, isotropic and anisotropic, and the
@@ -48,7 +48,8 @@ def test_box(B, oracle, shape, w):
     assert err(out, oracle.box_filter_oracle(a, *w)) <= TOL
 
 
-@pytest.mark.parametrize("fwhm", [(3, 3, 3), (2, 3, 3), (7, 3, 3), (1, 5, 3), (0, 3, 0), (12.9, 1, 1)], ids=str)
+@pytest.mark.parametrize("fwhm", [(3, 3, 3), (2, 3, 3), (7, 3, 3), (1, 5, 3), (0, 3, 0), (12.9, 1, 1), (5, 5, 5), (7, 7, 7), (5, 7, 3), (3, 3, 7)],
+                         ids=str)
 @pytest.mark.parametrize("shape", SHAPES, ids=IDS)
 def test_gaussian_axis_aligned(B, oracle, shape, fwhm):
     """theta = 0: separable path; paper FWHM 1..7 and the library limit."""
