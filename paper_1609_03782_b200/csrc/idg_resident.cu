@@ -246,7 +246,12 @@ __global__ void __launch_bounds__(kThreads, 1) idg_resident_kernel(const __grid_
     // Small blocks (the single-cube interactive case): at most one item per warp and two inbound
     // entries per thread.  Everything that does not change from one iteration to the next is worked out once, and a
     // warp runs the loop built for its number of cells.
-    const bool small = nwitems <= kThreads / 32 && n_in <= 2 * kThreads && A.ls <= kMaxChunk;
+    // The choice must be the SAME for every CTA of the grid (the two paths hand faces over differently: only the
+    // large-block path raises and waits for the per-face flags), so it is taken on the NOMINAL block extents, not on
+    // this CTA's -- a ragged last block is smaller and would otherwise pick the other path than its neighbours.
+    const int nom_items = ((nx4 * A.by + 31) / 32) * ((A.bz + A.ls - 1) / A.ls);
+    const int nom_in = 2 * nx4 * (A.by + A.bz);
+    const bool small = nom_items <= kThreads / 32 && nom_in <= 2 * kThreads && A.ls <= kMaxChunk;
     if (small) {
         const Item I = decode(warp < nwitems ? warp : 0);
         const int cnt = warp < nwitems ? I.ze - I.zs : 0;

@@ -515,13 +515,14 @@ def test_auto_plan_by_size(B):
 
 @pytest.mark.parametrize("shape,nb", [((67, 100, 100), 1), ((5, 9, 8), 1), ((1, 1, 8), 1), ((3, 300, 16), 1), ((200, 3, 24), 1),
                                       ((64, 128, 128), 3), ((67, 100, 100), 7), ((20, 24, 520), 2), ((128, 128, 128), 1),
-                                      ((33, 77, 132), 5)],
+                                      ((33, 77, 132), 5), ((13, 150, 268), 1), ((10, 150, 268), 1)],
                          ids=lambda v: "x".join(map(str, v[::-1])) if isinstance(v, tuple) else f"b{v}")
 def test_resident_kernel_is_bitwise_equal_to_the_naive_kernel_and_repeatable(B, shape, nb):
     """idg_resident_kernel: blocks of the cube stay in shared memory for all iterations, faces travel through mailboxes
     with the iteration tag packed into every word.  Same arithmetic as every other kernel -> bit-identical to the
     one-thread-per-voxel kernel, on every run (a face read before it arrived, or a mailbox overwritten too early, would
-    show as a differing voxel), for ragged blocks, one to several waves of cubes, per-cube iteration counts (0 included),
+    show as a differing voxel), for ragged blocks (268 x 150 x 13: the last z block is small enough for the small-block
+    path while its neighbours are not -- every CTA must take the same path), one to several waves of cubes, per-cube iteration counts (0 included),
     in place, and for the gradient-driven variant."""
     g = torch.Generator(device="cuda").manual_seed(5)
     x = torch.randn((nb,) + shape, device="cuda", generator=g) * 2.0
