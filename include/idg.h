@@ -48,7 +48,8 @@ enum {
     IDG_ERR_PARAM = -4,            /* K <= 0 or NaN; tau, Cj < 0; rms <= 0; non-finite (K = +inf is allowed) */
     IDG_ERR_WORKSPACE = -5,        /* workspace NULL, too small or not 256-byte aligned */
     IDG_ERR_OVERLAP = -6,          /* cube/out/workspace partially overlap */
-    IDG_ERR_OPTION = -7            /* unknown option key or value out of range */
+    IDG_ERR_OPTION = -7,           /* unknown option key or value out of range */
+    IDG_ERR_STATIC_LIMIT = -8      /* idg_gaussian_filter_static: the kernel does not fit the static scratch array */
 };
 
 /*
@@ -176,6 +177,25 @@ int idg_box_filter(const float *cube, int nx, int ny, int nz, int wx, int wy, in
  */
 int idg_gaussian_filter(const float *cube, int nx, int ny, int nz, float fwhm_x, float fwhm_y, float fwhm_z,
                         float theta_x, float theta_y, float theta_z, float *out, void *stream);
+
+/*
+ * No-allocation variant of the ROTATED Gaussian filter (Eq. 3), for callers that cannot call cudaMalloc: code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid allocation.  As idg_gaussian_filter with a rotation (same
+ * readings, same kernel, same result), but the (2r+1)^3 kernel weights live in a static device array inside the library
+ * instead of a stream-ordered temporary: the call runs no cudaMalloc, cudaFree or other allocating routine.
+ *   limit     support radius r <= 9, i.e. 19^3 floats = 27 436 bytes, held by every GPU that loads the library until the
+ *             process exits (FWHM <= 7.4 voxels: every FWHM of the paper).  A larger kernel (which idg_gaussian_filter
+ *             takes up to r = 10) returns IDG_ERR_STATIC_LIMIT; nothing is enqueued.
+ *   angles    at least one must be non-zero; all zero returns IDG_ERR_PARAM (the separable path of idg_gaussian_filter
+ *             has no scratch and allocates nothing as it is).
+ *   sharing   every call on a device uses the ONE array and overwrites what the previous call left there, in stream
+ *             order.  Calls that overlap on the GPU (different streams not ordered by events, several host threads)
+ *             race on it and are not supported.  Nothing in it has to start at zero.
+ *   cube [device] nx*ny*nz fp32;  out [device] nx*ny*nz fp32, must not overlap cube.  Other errors as idg_gaussian_filter.
+ *   idg_last_launch_count / idg_last_plan are not updated by this call.
+ */
+int idg_gaussian_filter_static(const float *cube, int nx, int ny, int nz, float fwhm_x, float fwhm_y, float fwhm_z,
+                               float theta_x, float theta_y, float theta_z, float *out, void *stream);
 
 /*
  * Host-only: support radii (rx, ry, rz) idg_gaussian_filter would use, or IDG_ERR_PARAM.

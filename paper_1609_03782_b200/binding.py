@@ -26,7 +26,7 @@ SYMBOLS = ("idg_version", "idg_status_string", "idg_params_check", "idg_workspac
            "idg_set_option", "idg_get_option", "idg_last_launch_count", "idg_last_plan",
            "idg_box_filter", "idg_gaussian_filter", "idg_gaussian_radii",
            "idg_mask_sums", "idg_cube_stats", "idg_quality", "idg_filter_pm",
-           "idg_wavelet_transform", "idg_wavelet_filter", "idg_histogram", "idg_release_temporaries", "idg_stats_rms")
+           "idg_wavelet_transform", "idg_wavelet_filter", "idg_histogram", "idg_release_temporaries", "idg_stats_rms", "idg_gaussian_filter_static")
 WAVELET_HAAR, WAVELET_LEGALL53 = 0, 1
 
 
@@ -108,6 +108,8 @@ def lib() -> ctypes.CDLL:
         L.idg_box_filter.argtypes = [fp, i, i, i, i, i, i, fp, vp]
         L.idg_gaussian_filter.restype = i
         L.idg_gaussian_filter.argtypes = [fp, i, i, i, f, f, f, f, f, f, fp, vp]
+        L.idg_gaussian_filter_static.restype = i
+        L.idg_gaussian_filter_static.argtypes = [fp, i, i, i, f, f, f, f, f, f, fp, vp]
         L.idg_gaussian_radii.restype = i
         L.idg_gaussian_radii.argtypes = [f, f, f, f, f, f, ctypes.POINTER(ctypes.c_int)]
         rp, d, dptr = ctypes.POINTER(IdgRoi), ctypes.c_double, ctypes.POINTER(ctypes.c_double)
@@ -298,6 +300,22 @@ def idg_gaussian_filter(cube: torch.Tensor, fwhm: Sequence[float], theta: Sequen
     _check(lib().idg_gaussian_filter(_dev(cube, "cube"), nx, ny, nz, float(fwhm[0]), float(fwhm[1]),
                                      float(fwhm[2]), float(theta[0]), float(theta[1]), float(theta[2]),
                                      _dev(out, "out"), _stream(stream)))
+    return out
+
+
+def idg_gaussian_filter_static(cube: torch.Tensor, fwhm: Sequence[float], theta: Sequence[float],
+                               out: Optional[torch.Tensor] = None,
+                               stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """idg_gaussian_filter_static: the rotated Gaussian filter with its weights in the library's static device array
+    (no allocation inside the call when `out` is given; support radius <= 9, else IdgError status -8)."""
+    if cube.dim() != 3:
+        raise ValueError("cube must be [nz, ny, nx]")
+    nz, ny, nx = cube.shape
+    if out is None:
+        out = torch.empty_like(cube)
+    _check(lib().idg_gaussian_filter_static(_dev(cube, "cube"), nx, ny, nz, float(fwhm[0]), float(fwhm[1]),
+                                            float(fwhm[2]), float(theta[0]), float(theta[1]), float(theta[2]),
+                                            _dev(out, "out"), _stream(stream)))
     return out
 
 

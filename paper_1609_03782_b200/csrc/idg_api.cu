@@ -301,6 +301,7 @@ const char *idg_status_string(int status)
     case IDG_ERR_WORKSPACE: return "workspace missing, too small or misaligned";
     case IDG_ERR_OVERLAP: return "buffers overlap";
     case IDG_ERR_OPTION: return "unknown option or value out of range";
+    case IDG_ERR_STATIC_LIMIT: return "kernel larger than the static scratch array of idg_gaussian_filter_static (radius > 9)";
     default: return status > 0 ? cudaGetErrorString((cudaError_t)status) : "unknown status";
     }
 }

@@ -34,7 +34,7 @@ def test_header_symbols_are_exported(binding):
 def test_version_and_status_strings(binding):
     assert binding.idg_version() == 10100
     assert binding.status_string(0) == "ok"
-    for s in range(-7, 0):
+    for s in range(-8, 0):
         assert binding.status_string(s) not in ("", "unknown status")
 
 
