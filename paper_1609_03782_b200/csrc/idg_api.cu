@@ -117,8 +117,10 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
                               (kernel == 0 || kernel == 5) &&
                               idg::resident_plan(nx, ny, nz, batch, max_n, mail_bytes, idg::device_sm_count(), &rplan);
     if (kernel == 5 && !can_resident) kernel = 0;
-    // Measured (profiles/r2a_notes.md): faster than kernel 3 when the whole call fits on chip at once (one wave).
-    if (kernel == 0 && can_resident && fuse == 0 && rplan.cubes >= batch) kernel = 5;
+    // Measured (profiles/r2a_notes.md): faster than kernel 3 when the whole call fits on chip at once (one wave) AND the
+    // blocks are small enough for the kernel's small-block path (up to ~1.3 Mvoxel: 30 against 40 us on 100 x 100 x 67,
+    // 37 against 43 on 128 x 128 x 64); with larger blocks kernel 3 at T = 4 wins by 6-25 % (160 x 160 x 64 .. 256 x 256 x 40).
+    if (kernel == 0 && can_resident && fuse == 0 && rplan.cubes >= batch && rplan.small) kernel = 5;
     if (kernel == 0) {
         // Measured on B200 (profiles/r1g_notes.md, r1h_notes.md): the z-chunked TMA kernel everywhere it applies.
         // Four fused iterations per launch (one 8-warp CTA per SM) move a quarter of the DRAM bytes of an un-fused

@@ -134,6 +134,7 @@ struct ResidentPlan {
     int cubes;              // cubes per launch (wave)
     int words;              // 64-bit mailbox words per (block, parity)
     size_t smem;            // dynamic shared memory per CTA
+    bool small;             // the kernel will take its small-block path (one item per warp, <= 2 inbound entries per thread)
 };
 constexpr size_t kResidentMailBytes = (size_t)32 << 20;       // mailbox region reserved in the workspace
 constexpr size_t kResidentMaxCubeVoxels = (size_t)4 << 20;     // larger cubes cannot be held on chip

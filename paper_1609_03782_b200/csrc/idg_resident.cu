@@ -461,7 +461,10 @@ bool search_plan(int nx, int ny, int nz, int batch, int max_n, size_t mail_bytes
             const double cost = waves * (max_n * iter + io);
             if (best < 0 || cost < best) {
                 best = cost;
-                bp = ResidentPlan{ty, tz, by, bz, ls_best, cubes, (int)words, smem};
+                // the kernel's own predicate (nominal block extents; idg_resident_kernel: `small`)
+                const int nom_items = ((nx4 * by + 31) / 32) * ((bz + ls_best - 1) / ls_best);
+                const bool small = nom_items <= kThreads / 32 && 2 * nx4 * (by + bz) <= 2 * kThreads && ls_best <= kMaxChunk;
+                bp = ResidentPlan{ty, tz, by, bz, ls_best, cubes, (int)words, smem, small};
             }
         }
     }

@@ -498,12 +498,17 @@ def test_cooperative_launch_batched_mixed_iteration_counts(B, oracle):
 
 def test_auto_plan_by_size(B):
     """Auto plan: the resident kernel (cube on chip for the whole call, one cooperative launch) when the whole call fits
-    on chip at once; kernel 3 for larger cubes and batches; option COOP = 2 still folds kernel 3's rounds."""
+    on chip at once with small blocks (up to ~1.3 Mvoxel); kernel 3 for larger cubes and batches; option COOP = 2 still
+    folds kernel 3's rounds."""
     set_plan(B, (0, 0))
     B.idg_filter(torch.zeros(67, 100, 100, device="cuda"), 10)
     assert "idg_resident_kernel" in B.idg_last_plan() and B.idg_last_launch_count() == 1
     B.idg_filter(torch.zeros(128, 512, 512, device="cuda"), 8)
     assert "idg_tma_kernel" in B.idg_last_plan() and B.idg_last_launch_count() == 2
+    B.idg_filter(torch.zeros(64, 128, 128, device="cuda"), 10)       # still small blocks
+    assert "idg_resident_kernel" in B.idg_last_plan()
+    B.idg_filter(torch.zeros(64, 160, 160, device="cuda"), 10)       # fits on chip, but with large blocks: kernel 3 is faster
+    assert "idg_tma_kernel" in B.idg_last_plan()
     B.idg_filter_batched(torch.zeros(16, 67, 100, 100, device="cuda"), 10, [B.Params()] * 16)
     assert "idg_tma_kernel" in B.idg_last_plan()
     B.idg_filter(torch.zeros(8, 16, 18, device="cuda"), 3)           # nx % 4 != 0
