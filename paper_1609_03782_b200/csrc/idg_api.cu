@@ -450,7 +450,24 @@ int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
     if (slabs > kMaxSlabs) slabs = kMaxSlabs;
     if (slabs > nz) slabs = nz;
     const size_t plane_b = (size_t)nx * ny * sizeof(float);
-    const int zs = (nz + slabs - 1) / slabs;
+    // Slab boundaries.  Nothing can be downloaded before the first slab and its halo have been uploaded and filtered, and
+    // that lag adds to the total download time: the first slab is a quarter as thick as the others (from 4 slabs on;
+    // measured 0.91 of the copy-only floor against 0.89-0.90 with equal slabs; a thin last slab as well gave nothing).
+    int zb[kMaxSlabs + 1];
+    {
+        const int zs_u = (nz + slabs - 1) / slabs;
+        const int first = slabs >= 4 ? (zs_u / 4 > 1 ? zs_u / 4 : 1) : zs_u;
+        zb[0] = 0;
+        for (int i = 1; i <= slabs; ++i) {
+            long long z = slabs >= 4 ? first + ((long long)(nz - first) * (i - 1) + (slabs - 2)) / (slabs - 1)
+                                     : (long long)i * zs_u;
+            zb[i] = z < nz ? (int)z : nz;
+        }
+        zb[slabs] = nz;
+    }
+    int zs = 1;
+    for (int i = 0; i < slabs; ++i)
+        if (zb[i + 1] - zb[i] > zs) zs = zb[i + 1] - zb[i];                  // the thickest slab
     const int max_planes = zs + 2 * n_iter < nz ? zs + 2 * n_iter : nz;
     const size_t slab_al = align_up((size_t)max_planes * plane_b);
     const size_t slab_ws = idg_workspace_bytes(nx, ny, max_planes, 1);
@@ -469,8 +486,8 @@ int idg_filter_host(const float *cube_host, int nx, int ny, int nz, int n_iter,
         if (e == cudaSuccess) e = cudaStreamWaitEvent(s_h2d, ev_begin, 0);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(s_d2h, ev_begin, 0);
         for (int sl = 0; sl < slabs && e == cudaSuccess && rc == IDG_OK; ++sl) {
-            const int z0 = sl * zs, z1 = z0 + zs < nz ? z0 + zs : nz;
-            if (z0 >= z1) break;
+            const int z0 = zb[sl], z1 = zb[sl + 1];
+            if (z0 >= z1) continue;
             const int lo = z0 - n_iter > 0 ? z0 - n_iter : 0, hi = z1 + n_iter < nz ? z1 + n_iter : nz;
             if (hi > copied) {
                 e = cudaMemcpyAsync((char *)d_in + (size_t)copied * plane_b, (const char *)cube_host + (size_t)copied * plane_b,
