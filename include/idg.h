@@ -86,7 +86,7 @@ unsigned idg_params_check(const idg_params *params /*[host]*/);
  * pitch rounded up to 16 bytes, on which the TMA-fed kernel runs) plus a small
  * parameter table, the 256-byte block holding the
  * arrival counter of the cooperative single-launch path and, for cubes the resident
- * kernel can take (nx % 4 == 0, at most 4 Mi voxels), 32 MB of mailboxes for the
+ * kernel can take (nx >= 8, at most 4 Mi voxels), 32 MB of mailboxes for the
  * block faces.  0 on invalid dimensions.  A batch of more than ~2000 cubes uploads
  * its parameter table from pageable memory, which may synchronise the host.
  */
@@ -293,13 +293,15 @@ int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, i
 /*
  * Tuning knobs of the CALLING HOST THREAD (tests and benchmarks; defaults give the fastest plan): an option set by
  * one thread affects the calls that thread makes afterwards and no other thread's.
- *   IDG_OPT_KERNEL   0 auto (the resident kernel 5 when the whole call fits in the SMs' shared memory at once, else
+ *   IDG_OPT_KERNEL   0 auto (the resident kernel 5 when the whole call fits in the SMs' shared memory at once in small
+ *                    blocks -- cubes of up to ~1.3 Mvoxel --, else
  *                    kernel 3 wherever nx % 4 == 0 and the buffers are 16-byte aligned) | 1 naive (one thread per
  *                    voxel) | 2 tiled z-streaming kernel (global loads) | 3 tiled z-streaming kernel fed by TMA (the
  *                    fast path for large cubes) | 4 (retired: runs kernel 3) | 5 resident kernel: blocks of
  *                    the cube(s) stay in shared memory for all iterations of the call, block faces are exchanged
  *                    through mailboxes in the workspace, one cooperative launch per wave of cubes (cubes of up to
- *                    4 Mi voxels with nx % 4 == 0, nx >= 8; otherwise the auto plan).  Reference filters: 1 = the
+ *                    4 Mi voxels with nx >= 8, any alignment: rows are padded to float4 on chip; otherwise the auto
+ *                    plan).  Reference filters: 1 = the
  *                    general separable kernel also where the TMA-fed one applies.  Wavelets: see idg_wavelet_filter
  *   IDG_OPT_FUSE     0 auto (4, or 2 for full-GPU workloads of cubes thinner than 100 planes) | 1..4 = diffusion
  *                    iterations fused per launch (kernels 2-4)

@@ -31,9 +31,9 @@ bool voxel_count(int nx, int ny, int nz, int batch, size_t *n_one)
     return true;
 }
 
-// Shapes the resident kernel can take (float4 rows, a cube small enough to sit in the SMs' shared memory): the
-// workspace then carries the mailbox region.
-bool resident_shape(int nx, size_t N) { return nx % 4 == 0 && N <= idg::kResidentMaxCubeVoxels; }
+// Shapes the resident kernel can take (a cube small enough to sit in the SMs' shared memory; any nx >= 8, rows are
+// padded to float4 on chip): the workspace then carries the mailbox region.
+bool resident_shape(int nx, size_t N) { return nx >= 8 && N <= idg::kResidentMaxCubeVoxels; }
 
 // Bytes of one pitched copy of a batch (row pitch = nx rounded up to a multiple of 4 floats = 16 bytes).
 size_t pitched_bytes(int nx, int ny, int nz, int batch)
@@ -113,8 +113,7 @@ int run(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter
     bool pitched = false;
     // Small cubes and interactive batches: everything on chip for the whole call (profiles/r2a_notes.md).
     idg::ResidentPlan rplan;
-    const bool can_resident = mail_bytes > 0 && max_n > 0 && (((uintptr_t)cubes | (uintptr_t)out) & 15u) == 0 &&
-                              (kernel == 0 || kernel == 5) &&
+    const bool can_resident = mail_bytes > 0 && max_n > 0 && (kernel == 0 || kernel == 5) &&
                               idg::resident_plan(nx, ny, nz, batch, max_n, mail_bytes, idg::device_sm_count(), &rplan);
     if (kernel == 5 && !can_resident) kernel = 0;
     // Measured (profiles/r2a_notes.md): faster than kernel 3 when the whole call fits on chip at once (one wave) AND the

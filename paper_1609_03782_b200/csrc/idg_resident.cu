@@ -44,8 +44,10 @@ struct ResArgs {
     int ty, tz;                     // blocks per cube along y, z
     int by, bz;                     // nominal block extents (the last block of an axis may be smaller)
     int ls;                         // z cells per work item
-    int words;                      // 64-bit words per (block, parity): 2 nx (by + bz) of faces + 8 (4 flags)
-    unsigned m_nx4;                 // ceil(2^32 / (nx / 4)): division by multiplication
+    int words;                      // 64-bit words per (block, parity): 8 nx4 (by + bz) of faces + 8 (4 flags)
+    unsigned m_nx4;                 // ceil(2^32 / nx4), nx4 = ceil(nx / 4): division by multiplication
+    int tail;                       // nx % 4: voxels in the last float4 of a row (0: all four)
+    int unal;                       // rows of the cubes are not 16-byte aligned (tail != 0 or odd base pointers): scalar global access
 };
 
 __device__ __forceinline__ void st_relaxed_v2(unsigned long long *p, unsigned long long a, unsigned long long b)
@@ -96,7 +98,8 @@ struct Item {
 // pm / p0: the column's cells in planes z-1 and z; on return those of planes z+CH-1 and z+CH.
 template <int CH, bool PM>
 __device__ __forceinline__ void chunk(const float *cur, float *nxt, int off, int PP, int RP, F4 &pm, F4 &p0, bool first,
-                                      bool last, bool lds_l, bool lds_r, bool valid, const Consts &kc, F4 (&o)[CH])
+                                      bool last, bool lds_l, bool lds_r, bool valid, const Consts &kc, F4 (&o)[CH],
+                                      int tail)
 {
     F4 pl[CH + 2], ym[CH], yp[CH];
     float l[CH], r[CH];
@@ -119,6 +122,14 @@ __device__ __forceinline__ void chunk(const float *cur, float *nxt, int off, int
     for (int k = 0; k < CH; ++k)
         o[k] = update4<PM>(pl[k + 1], first ? pl[k + 1].x : l[k], last ? pl[k + 1].w : r[k], ym[k], yp[k], pl[k],
                            pl[k + 2], kc);
+    if (tail && last) {             // nx % 4 != 0: the pad components of a row's last float4 repeat the last voxel --
+#pragma unroll                      // the replicated x face (reading R1) of the next iteration
+        for (int k = 0; k < CH; ++k) {
+            if (tail == 1) o[k].y = o[k].z = o[k].w = o[k].x;
+            else if (tail == 2) o[k].z = o[k].w = o[k].y;
+            else o[k].w = o[k].z;
+        }
+    }
     if (valid) {
 #pragma unroll
         for (int k = 0; k < CH; ++k) sts4(nxt + off + k * PP, o[k]);
@@ -127,19 +138,22 @@ __device__ __forceinline__ void chunk(const float *cur, float *nxt, int off, int
     p0 = pl[CH + 1];
 }
 
-template <bool PM>
+// UNAL: rows of the cubes are not 16-byte aligned (nx % 4 != 0 or odd base pointers): scalar global access, and the pad
+// components of a row's last float4 are kept equal to the last voxel.  The aligned instantiation has none of that.
+template <bool PM, bool UNAL>
 __global__ void __launch_bounds__(kThreads, 1) idg_resident_kernel(const __grid_constant__ ResArgs A)
 {
+    const int tail = UNAL ? A.tail : 0;
     extern __shared__ __align__(16) float smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int s = blockIdx.x;
     const int iy = s % A.ty, iz = (s / A.ty) % A.tz, cube = s / (A.ty * A.tz);
     const CubeParams prm = A.tab ? A.tab[cube] : A.one;
-    const int nx = A.nx, nx4 = nx >> 2;
+    const int nx = A.nx, nx4 = (nx + 3) >> 2;              // float4 columns of a (padded) row
     const unsigned mx4 = A.m_nx4;
     const int y0 = iy * A.by, h = min(A.by, A.ny - y0);
     const int z0 = iz * A.bz, d = min(A.bz, A.nz - z0);
-    const int RP = nx, PP = (A.by + 2) * nx;                       // row / plane pitch in floats
+    const int RP = 4 * nx4, PP = (A.by + 2) * RP;                  // row / plane pitch in floats (rows padded to float4)
     const int buf = (A.bz + 2) * PP + 8;                             // one copy (+ slack for the x reads at the ends)
     float *cur = smem + 4, *nxt = smem + 4 + buf;
     // neighbours: the block holding my y-1 / y+h rows and my z-1 / z+d planes (-1: a true cube face)
@@ -162,7 +176,17 @@ __global__ void __launch_bounds__(kThreads, 1) idg_resident_kernel(const __grid_
         for (int i = tid; i < cells; i += kThreads) {
             const int r = fdiv(i, mx4), x4 = i - r * nx4, zz = r / (h + 2), y = r - zz * (h + 2) - 1, z = zz - 1;
             const int gy = min(max(y0 + y, 0), A.ny - 1), gz = min(max(z0 + z, 0), A.nz - 1);
-            const float4 v = __ldg(reinterpret_cast<const float4 *>(src + (size_t)gz * plane_g + (size_t)gy * nx) + x4);
+            const float *row = src + (size_t)gz * plane_g + (size_t)gy * nx;
+            float4 v;
+            if (!UNAL) {
+                v = __ldg(reinterpret_cast<const float4 *>(row) + x4);
+            } else {                    // scalar loads; components beyond the row repeat its last voxel
+                const int x = 4 * x4;
+                v.x = __ldg(row + x);
+                v.y = __ldg(row + min(x + 1, nx - 1));
+                v.z = __ldg(row + min(x + 2, nx - 1));
+                v.w = __ldg(row + min(x + 3, nx - 1));
+            }
             *reinterpret_cast<float4 *>(cur + (z + 1) * PP + (y + 1) * RP + 4 * x4) = v;
         }
     }
@@ -207,8 +231,8 @@ __global__ void __launch_bounds__(kThreads, 1) idg_resident_kernel(const __grid_
         int z = I.zs;
         F4 oM[kMaxChunk], o1[1];
         for (; z + kMaxChunk <= I.ze; z += kMaxChunk, off += kMaxChunk * PP)
-            chunk<kMaxChunk, PM>(cur, nxt, off, PP, RP, pm, p0, first, last, lds_l, lds_r, I.valid, kc, oM);
-        for (; z < I.ze; ++z, off += PP) chunk<1, PM>(cur, nxt, off, PP, RP, pm, p0, first, last, lds_l, lds_r, I.valid, kc, o1);
+            chunk<kMaxChunk, PM>(cur, nxt, off, PP, RP, pm, p0, first, last, lds_l, lds_r, I.valid, kc, oM, tail);
+        for (; z < I.ze; ++z, off += PP) chunk<1, PM>(cur, nxt, off, PP, RP, pm, p0, first, last, lds_l, lds_r, I.valid, kc, o1, tail);
         if (!I.valid) return;
         // my own face cells (read back from `nxt`: this thread wrote them)
         if (I.y == 0 || I.y == h - 1) {
@@ -272,7 +296,7 @@ __global__ void __launch_bounds__(kThreads, 1) idg_resident_kernel(const __grid_
                 if (CH > 0) {
                     F4 o[CH > 0 ? CH : 1];
                     F4 pm = lds4(cur + I.off - PP), p0 = lds4(cur + I.off);
-                    chunk<(CH > 0 ? CH : 1), PM>(cur, nxt, I.off, PP, RP, pm, p0, first, last, lds_l, lds_r, I.valid, kc, o);
+                    chunk<(CH > 0 ? CH : 1), PM>(cur, nxt, I.off, PP, RP, pm, p0, first, last, lds_l, lds_r, I.valid, kc, o, tail);
                     if (I.valid) {
 #pragma unroll
                         for (int k = 0; k < CH; ++k) {
@@ -374,7 +398,16 @@ __global__ void __launch_bounds__(kThreads, 1) idg_resident_kernel(const __grid_
         for (int i = tid; i < cells; i += kThreads) {
             const int r = fdiv(i, mx4), x4 = i - r * nx4, z = r / h, y = r - z * h;
             const float4 v = *reinterpret_cast<const float4 *>(cur + (z + 1) * PP + (y + 1) * RP + 4 * x4);
-            reinterpret_cast<float4 *>(dst + (size_t)(z0 + z) * plane_g + (size_t)(y0 + y) * nx)[x4] = v;
+            float *row = dst + (size_t)(z0 + z) * plane_g + (size_t)(y0 + y) * nx;
+            if (!UNAL) {
+                reinterpret_cast<float4 *>(row)[x4] = v;
+            } else {
+                const int x = 4 * x4;
+                row[x] = v.x;
+                if (x + 1 < nx) row[x + 1] = v.y;
+                if (x + 2 < nx) row[x + 2] = v.z;
+                if (x + 3 < nx) row[x + 3] = v.w;
+            }
         }
     }
 }
@@ -428,8 +461,8 @@ bool resident_plan(int nx, int ny, int nz, int batch, int max_n, size_t mail_byt
 namespace {
 bool search_plan(int nx, int ny, int nz, int batch, int max_n, size_t mail_bytes, int sms, ResidentPlan *out)
 {
-    if (nx % 4 != 0 || nx < 8 || sms < 1 || max_n < 1) return false;      // nx = 4: the division by multiplication needs nx / 4 > 1
-    const int nx4 = nx / 4;
+    if (nx < 8 || sms < 1 || max_n < 1) return false;      // (the division by multiplication needs nx4 > 1)
+    const int nx4 = (nx + 3) / 4, nxp = 4 * nx4;           // rows are padded to whole float4 in shared memory
     double best = -1.0;
     ResidentPlan bp{};
     for (int ty = 1; ty <= ny && ty <= sms; ++ty) {
@@ -438,11 +471,11 @@ bool search_plan(int nx, int ny, int nz, int batch, int max_n, size_t mail_bytes
         for (int tz = 1; tz <= nz && ty * tz <= sms; ++tz) {
             const int bz = (nz + tz - 1) / tz;
             if ((tz - 1) * bz >= nz) continue;
-            const size_t smem = 2 * ((size_t)(bz + 2) * (by + 2) * nx + 8) * sizeof(float);
+            const size_t smem = 2 * ((size_t)(bz + 2) * (by + 2) * nxp + 8) * sizeof(float);
             if (smem > kSmemBudget) continue;
             const int per_wave = sms / (ty * tz);                   // cubes per launch
             const int cubes = per_wave < batch ? per_wave : batch;
-            const size_t words = (size_t)2 * nx * (by + bz) + 8;      // faces + one arrival flag per face
+            const size_t words = (size_t)2 * nxp * (by + bz) + 8;     // faces + one arrival flag per face
             if ((size_t)cubes * ty * tz * 2 * words * 8 > mail_bytes) continue;
             const int waves = (batch + per_wave - 1) / per_wave;
             // a warp item = 32 columns x ls cells; pick the segment length that balances the 16 warps best
@@ -477,14 +510,17 @@ bool search_plan(int nx, int ny, int nz, int batch, int max_n, size_t mail_bytes
 cudaError_t launch_resident(const Launch &L, const ResidentPlan &P, unsigned long long *mail, cudaStream_t st,
                             int *launches)
 {
-    void (*kern)(ResArgs) = L.mode == 1 ? idg_resident_kernel<true> : idg_resident_kernel<false>;
+    const bool unal = (L.nx & 3) != 0 || (((uintptr_t)L.in | (uintptr_t)L.out) & 15u) != 0;
+    void (*kern)(ResArgs) = L.mode == 1 ? (unal ? idg_resident_kernel<true, true> : idg_resident_kernel<true, false>)
+                                        : (unal ? idg_resident_kernel<false, true> : idg_resident_kernel<false, false>);
     // function attribute and co-residency check once per (thread, device, variant, shared-memory size)
     struct Checked { int dev, mode; size_t smem; long slots; };
     thread_local Checked chk{-1, 0, 0, 0};
+    const int variant = L.mode * 2 + (unal ? 1 : 0);
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    if (chk.dev != dev || chk.mode != L.mode || chk.smem != P.smem) {
+    if (chk.dev != dev || chk.mode != variant || chk.smem != P.smem) {
         const DevInfo di = dev_info();
         if (!di.coop) return cudaErrorNotSupported;
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P.smem);
@@ -492,7 +528,7 @@ cudaError_t launch_resident(const Launch &L, const ResidentPlan &P, unsigned lon
         int per_sm = 0;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kThreads, P.smem);
         if (e != cudaSuccess) return e;
-        chk = Checked{dev, L.mode, P.smem, (long)per_sm * di.sms};
+        chk = Checked{dev, variant, P.smem, (long)per_sm * di.sms};
     }
     if ((long)P.ty * P.tz * P.cubes > chk.slots) return cudaErrorCooperativeLaunchTooLarge;
     const size_t N = (size_t)L.nx * (size_t)L.ny * (size_t)L.nz;
@@ -508,7 +544,10 @@ cudaError_t launch_resident(const Launch &L, const ResidentPlan &P, unsigned lon
         A.nx = L.nx; A.ny = L.ny; A.nz = L.nz;
         A.ty = P.ty; A.tz = P.tz; A.by = P.by; A.bz = P.bz; A.ls = P.ls;
         A.words = P.words;
-        A.m_nx4 = (unsigned)((0x100000000ull + (unsigned)(L.nx / 4) - 1) / (unsigned)(L.nx / 4));
+        const unsigned nx4 = (unsigned)((L.nx + 3) / 4);
+        A.m_nx4 = (unsigned)((0x100000000ull + nx4 - 1) / nx4);
+        A.tail = L.nx & 3;
+        A.unal = unal ? 1 : 0;
         void *args[1] = {(void *)&A};
         e = cudaLaunchCooperativeKernel((const void *)kern, dim3((unsigned)(P.ty * P.tz * nc)), dim3(kThreads), args,
                                         P.smem, st);

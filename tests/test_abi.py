@@ -103,12 +103,15 @@ def test_stats_rms(binding):
 
 
 def test_resident_shapes_reserve_mailboxes(binding):
-    """Cubes the resident kernel can take (nx % 4 == 0, <= 4 Mi voxels) carry 32 MB of mailboxes in the workspace."""
+    """Cubes the resident kernel can take (nx >= 8, <= 4 Mi voxels) carry 32 MB of mailboxes in the workspace."""
     small = binding.idg_workspace_bytes(100, 100, 67, 1)
     assert small >= 100 * 100 * 67 * 4 + (32 << 20)
-    # nx % 4 != 0: no mailboxes, three pitched copies (row pitch 104 floats) for kernel 3 instead of one scratch cube
+    # nx % 4 != 0: three pitched copies (row pitch 104 floats) for kernel 3 instead of one scratch cube, and the
+    # mailboxes as well (the resident kernel pads rows on chip)
     w = binding.idg_workspace_bytes(102, 100, 67, 1)
-    assert 3 * 104 * 100 * 67 * 4 <= w < 3 * 104 * 100 * 67 * 4 + (1 << 20)
+    assert 3 * 104 * 100 * 67 * 4 + (32 << 20) <= w < 3 * 104 * 100 * 67 * 4 + (33 << 20)
+    w = binding.idg_workspace_bytes(1023, 1023, 512, 1)             # too large for the chip: no mailboxes
+    assert 3 * 1024 * 1023 * 512 * 4 <= w < 3 * 1024 * 1023 * 512 * 4 + (1 << 20)
     assert binding.idg_workspace_bytes(1024, 1024, 512, 1) < 1024 * 1024 * 512 * 4 + (1 << 20)  # too large
 
 

@@ -511,8 +511,12 @@ def test_auto_plan_by_size(B):
     assert "idg_tma_kernel" in B.idg_last_plan()
     B.idg_filter_batched(torch.zeros(16, 67, 100, 100, device="cuda"), 10, [B.Params()] * 16)
     assert "idg_tma_kernel" in B.idg_last_plan()
-    B.idg_filter(torch.zeros(8, 16, 18, device="cuda"), 3)           # nx % 4 != 0
-    assert "idg_resident_kernel" not in B.idg_last_plan()
+    B.idg_filter(torch.zeros(67, 101, 101, device="cuda"), 10)       # nx % 4 != 0: rows are padded to float4 on chip
+    assert "idg_resident_kernel" in B.idg_last_plan()
+    B.idg_filter(torch.zeros(64, 300, 301, device="cuda"), 8)        # too large for the chip: kernel 3 on pitched copies
+    assert "pitched" in B.idg_last_plan()
+    B.idg_filter(torch.zeros(8, 16, 6, device="cuda"), 3)            # nx < 8: neither
+    assert "idg_naive_kernel" in B.idg_last_plan()
     set_plan(B, (3, 3), coop=2)
     B.idg_filter(torch.zeros(67, 100, 100, device="cuda"), 10)
     assert "idg_tma_coop_kernel" in B.idg_last_plan() and B.idg_last_launch_count() == 1
@@ -520,7 +524,9 @@ def test_auto_plan_by_size(B):
 
 @pytest.mark.parametrize("shape,nb", [((67, 100, 100), 1), ((5, 9, 8), 1), ((1, 1, 8), 1), ((3, 300, 16), 1), ((200, 3, 24), 1),
                                       ((64, 128, 128), 3), ((67, 100, 100), 7), ((20, 24, 520), 2), ((128, 128, 128), 1),
-                                      ((33, 77, 132), 5), ((13, 150, 268), 1), ((10, 150, 268), 1)],
+                                      ((33, 77, 132), 5), ((13, 150, 268), 1), ((10, 150, 268), 1),
+                                      ((67, 101, 101), 1), ((9, 37, 33), 3), ((20, 30, 9), 2), ((13, 150, 270), 1),
+                                      ((16, 40, 127), 2), ((64, 129, 130), 1), ((5, 7, 11), 1)],
                          ids=lambda v: "x".join(map(str, v[::-1])) if isinstance(v, tuple) else f"b{v}")
 def test_resident_kernel_is_bitwise_equal_to_the_naive_kernel_and_repeatable(B, shape, nb):
     """idg_resident_kernel: blocks of the cube stay in shared memory for all iterations, faces travel through mailboxes
@@ -528,7 +534,8 @@ def test_resident_kernel_is_bitwise_equal_to_the_naive_kernel_and_repeatable(B, 
     one-thread-per-voxel kernel, on every run (a face read before it arrived, or a mailbox overwritten too early, would
     show as a differing voxel), for ragged blocks (268 x 150 x 13: the last z block is small enough for the small-block
     path while its neighbours are not -- every CTA must take the same path), one to several waves of cubes, per-cube iteration counts (0 included),
-    in place, and for the gradient-driven variant."""
+    in place, for the gradient-driven variant, and for nx % 4 != 0 (rows padded to float4 in shared memory, the pad
+    components of the last float4 repeat the last voxel = the replicated x face; scalar global loads and stores)."""
     g = torch.Generator(device="cuda").manual_seed(5)
     x = torch.randn((nb,) + shape, device="cuda", generator=g) * 2.0
     ps = [B.Params(K=1.0 + 0.25 * b, tau=0.03, cx=5.0, cy=4.0, cz=6.0, rms=1.0) for b in range(nb)]
@@ -577,7 +584,7 @@ def test_unaligned_rows_run_the_tma_kernel_on_pitched_copies(B, oracle, nx):
     big = torch.randn((40, 120, nx), device="cuda", generator=g)
     if big.numel() >= 100_000:
         out = B.idg_filter(big, 6, ps[0])
-        assert "pitched" in B.idg_last_plan()
+        assert "pitched" in B.idg_last_plan() or "idg_resident_kernel" in B.idg_last_plan()
         set_plan(B, (1, 0))
         assert torch.equal(out, B.idg_filter(big, 6, ps[0]))
     want = oracle.idg_filter_oracle(x[0].cpu().numpy(), 9, **ps[0].f32())
