@@ -294,8 +294,8 @@ int idg_wavelet_filter(const float *cube, int nx, int ny, int nz, int wavelet, i
  * Tuning knobs of the CALLING HOST THREAD (tests and benchmarks; defaults give the fastest plan): an option set by
  * one thread affects the calls that thread makes afterwards and no other thread's.
  *   IDG_OPT_KERNEL   0 auto (the resident kernel 5 when the whole call fits in the SMs' shared memory at once in small
- *                    blocks -- cubes of up to ~1.3 Mvoxel --, else
- *                    kernel 3 wherever nx % 4 == 0 and the buffers are 16-byte aligned) | 1 naive (one thread per
+ *                    blocks -- cubes of up to ~1.3 Mvoxel --, else kernel 3: directly where nx % 4 == 0 and the buffers
+ *                    are 16-byte aligned, on pitched copies in the workspace otherwise) | 1 naive (one thread per
  *                    voxel) | 2 tiled z-streaming kernel (global loads) | 3 tiled z-streaming kernel fed by TMA (the
  *                    fast path for large cubes) | 4 (retired: runs kernel 3) | 5 resident kernel: blocks of
  *                    the cube(s) stay in shared memory for all iterations of the call, block faces are exchanged
