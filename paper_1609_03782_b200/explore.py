@@ -3,8 +3,9 @@
     python -m paper_1609_03782_b200.explore [--snr 22] [--seed 1001] [--nmax 40] [--filter idg|pm]
 
 For a ModelB-like synthetic cube (BASELINE.json configs[1]) the intensity-driven gradient filter is run for
-every K of the sweep and n = 1 .. nmax (incrementally: f(I, n+1) = f(f(I, n), 1), DESIGN.md pin P11), and after
-every iteration the quality diagnostics are evaluated on the device: rms of the filtered cube over signal-free
+every K of the sweep -- all K as one batched call with per-cube parameters -- up to n = nmax, incrementally from one
+reported n to the next (f(I, n+m) = f(f(I, n), m), DESIGN.md pin P11; the iterations in between are fused on the
+device), and at every reported n the quality diagnostics are evaluated on the device: rms of the filtered cube over signal-free
 channels (idg_cube_stats), the masked sums over the ROI (idg_mask_sums) and F, sigma_F, F_M (idg_quality,
 Eq. 12-18).  Prints one line per (K, n) of interest and the best run by F, like Table 1 / Table 3 of the paper.
 Everything numerical runs in the library's CUDA kernels; this module only marshals arguments.
@@ -34,23 +35,32 @@ def explore(snr: float = 22.0, seed: int = 1001, nmax: int = 40, variant: str = 
     chan = np.abs(c.model).reshape(nz, -1).max(axis=1) > 0.05 * np.abs(c.model).max()
     z0, z1 = int(np.argmax(chan)), int(nz - np.argmax(chan[::-1]))
     roi = (0, nx, 0, ny, z0, z1)
-    ws = B.alloc_workspace(nx, ny, nz, 1)
-    step = B.idg_filter_pm if variant == "pm" else B.idg_filter
+    # all K values as ONE batch (idg_filter_batched, per-cube parameters), and the iterations between two reported n in
+    # one call (fused on the device): f(I, n + m) = f(f(I, n), m), DESIGN.md pin P11
+    ks = [float(K) for K in ks]
+    plist = [B.Params(K=K, rms=float(c.rms)) for K in ks]
+    cur = orig.unsqueeze(0).repeat(len(ks), 1, 1, 1).contiguous()
+    ws = B.alloc_workspace(nx, ny, nz, len(ks))
     sums = torch.empty(8, dtype=torch.float64, device="cuda")
     stats = torch.empty(8, dtype=torch.float64, device="cuda")
-    rows = []
-    for K in ks:
-        p = B.Params(K=float(K), rms=float(c.rms))
-        cur = orig.clone()
-        for n in range(1, nmax + 1):
-            step(cur, 1, p, out=cur, workspace=ws)
-            if n not in report:
-                continue
-            st = B.idg_cube_stats(cur, noise_roi, stats).cpu().numpy()
+    rows, done = [], 0
+    for n in sorted(m for m in set(report) | {nmax} if 1 <= m <= nmax):
+        if variant == "pm":                 # the gradient-driven variant has no batched entry point: cube by cube
+            ws1 = B.alloc_workspace(nx, ny, nz, 1)
+            for b, p in enumerate(plist):
+                B.idg_filter_pm(cur[b], n - done, p, out=cur[b], workspace=ws1)
+        else:
+            B.idg_filter_batched(cur, n - done, plist, out=cur, workspace=ws)
+        done = n
+        if n not in report:
+            continue
+        for b, K in enumerate(ks):
+            st = B.idg_cube_stats(cur[b], noise_roi, stats).cpu().numpy()
             rms_f = B.idg_stats_rms(st)[1]
-            s = B.idg_mask_sums(orig, cur, model, 3.0 * c.rms, 3.0 * rms_f, roi, sums).cpu().numpy()
+            s = B.idg_mask_sums(orig, cur[b], model, 3.0 * c.rms, 3.0 * rms_f, roi, sums).cpu().numpy()
             q = B.idg_quality(s, c.rms, rms_f)
-            rows.append({"K": float(K), "n": n, "rms_f": rms_f, **q})
+            rows.append({"K": K, "n": n, "rms_f": rms_f, **q})
+    rows.sort(key=lambda r: (r["K"], r["n"]))
     return rows
 
 
