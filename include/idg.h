@@ -122,6 +122,14 @@ int idg_filter_pm(const float *cube, int nx, int ny, int nz, int n_iter, const i
                   float *out, void *workspace, size_t workspace_bytes, void *stream);
 
 /*
+ * The gradient-driven variant for `batch` cubes in one call: arguments, layout and errors as idg_filter_batched,
+ * arithmetic as idg_filter_pm.
+ */
+int idg_filter_pm_batched(const float *cubes, int nx, int ny, int nz, int batch,
+                          const int *n_iter, int n_iter_all, const idg_params *params,
+                          float *out, void *workspace, size_t workspace_bytes, void *stream);
+
+/*
  * `batch` independent cubes of equal shape in one call (interactive parameter
  * exploration), each with its own parameters and
  * iteration count.

@@ -26,7 +26,7 @@ SYMBOLS = ("idg_version", "idg_status_string", "idg_params_check", "idg_workspac
            "idg_set_option", "idg_get_option", "idg_last_launch_count", "idg_last_plan",
            "idg_box_filter", "idg_gaussian_filter", "idg_gaussian_radii",
            "idg_mask_sums", "idg_cube_stats", "idg_quality", "idg_filter_pm",
-           "idg_wavelet_transform", "idg_wavelet_filter", "idg_histogram", "idg_release_temporaries", "idg_stats_rms", "idg_gaussian_filter_static")
+           "idg_wavelet_transform", "idg_wavelet_filter", "idg_histogram", "idg_release_temporaries", "idg_stats_rms", "idg_gaussian_filter_static", "idg_filter_pm_batched")
 WAVELET_HAAR, WAVELET_LEGALL53 = 0, 1
 
 
@@ -93,6 +93,8 @@ def lib() -> ctypes.CDLL:
         L.idg_filter_pm.argtypes = [fp, i, i, i, i, pp, fp, vp, sz, vp]
         L.idg_filter_batched.restype = i
         L.idg_filter_batched.argtypes = [fp, i, i, i, i, ip, i, pp, fp, vp, sz, vp]
+        L.idg_filter_pm_batched.restype = i
+        L.idg_filter_pm_batched.argtypes = [fp, i, i, i, i, ip, i, pp, fp, vp, sz, vp]
         L.idg_filter_host.restype = i
         L.idg_filter_host.argtypes = [fp, i, i, i, i, pp, fp, vp, sz, vp]
         L.idg_set_option.restype = i
@@ -231,8 +233,8 @@ def idg_filter_pm(cube: torch.Tensor, n_iter: int, params: Params = Params(),
 def idg_filter_batched(cubes: torch.Tensor, n_iter: Union[int, Sequence[int]],
                        params: Sequence[Params], out: Optional[torch.Tensor] = None,
                        workspace: Optional[torch.Tensor] = None,
-                       stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
-    """idg_filter_batched on a [B, nz, ny, nx] CUDA tensor with per-cube parameters."""
+                       stream: Optional[torch.cuda.Stream] = None, variant: str = "idg") -> torch.Tensor:
+    """idg_filter_batched (variant "pm": idg_filter_pm_batched) on a [B, nz, ny, nx] CUDA tensor with per-cube parameters."""
     if cubes.dim() != 4:
         raise ValueError("cubes must be [B, nz, ny, nx]")
     B, nz, ny, nx = cubes.shape
@@ -250,11 +252,18 @@ def idg_filter_batched(cubes: torch.Tensor, n_iter: Union[int, Sequence[int]],
             raise ValueError("one n_iter per cube")
         n_arr = (ctypes.c_int * B)(*[int(v) for v in n_iter])
         n_ptr, n_all = ctypes.cast(n_arr, ctypes.c_void_p), 0
-    rc = lib().idg_filter_batched(_dev(cubes, "cubes"), nx, ny, nz, B, n_ptr, n_all, arr,
-                                  _dev(out, "out"), workspace.data_ptr(), workspace.numel(),
-                                  _stream(stream))
+    fn = lib().idg_filter_pm_batched if variant == "pm" else lib().idg_filter_batched
+    rc = fn(_dev(cubes, "cubes"), nx, ny, nz, B, n_ptr, n_all, arr, _dev(out, "out"), workspace.data_ptr(),
+            workspace.numel(), _stream(stream))
     _check(rc)
     return out
+
+
+def idg_filter_pm_batched(cubes: torch.Tensor, n_iter: Union[int, Sequence[int]], params: Sequence[Params],
+                          out: Optional[torch.Tensor] = None, workspace: Optional[torch.Tensor] = None,
+                          stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """idg_filter_pm_batched: the gradient-driven variant (Eq. 5) on a [B, nz, ny, nx] CUDA tensor."""
+    return idg_filter_batched(cubes, n_iter, params, out, workspace, stream, variant="pm")
 
 
 def idg_filter_host(cube_host: torch.Tensor, n_iter: int, params: Params = Params(),

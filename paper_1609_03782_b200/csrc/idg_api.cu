@@ -351,6 +351,14 @@ int idg_filter_batched(const float *cubes, int nx, int ny, int nz, int batch, co
                (cudaStream_t)stream);
 }
 
+int idg_filter_pm_batched(const float *cubes, int nx, int ny, int nz, int batch, const int *n_iter,
+                          int n_iter_all, const idg_params *params, float *out, void *workspace,
+                          size_t workspace_bytes, void *stream)
+{
+    return run(cubes, nx, ny, nz, batch, n_iter, n_iter_all, params, out, workspace, workspace_bytes,
+               (cudaStream_t)stream, 1);
+}
+
 int idg_filter(const float *cube, int nx, int ny, int nz, int n_iter, const idg_params *params,
                float *out, void *stream)
 {

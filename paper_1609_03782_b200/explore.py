@@ -45,12 +45,8 @@ def explore(snr: float = 22.0, seed: int = 1001, nmax: int = 40, variant: str = 
     stats = torch.empty(8, dtype=torch.float64, device="cuda")
     rows, done = [], 0
     for n in sorted(m for m in set(report) | {nmax} if 1 <= m <= nmax):
-        if variant == "pm":                 # the gradient-driven variant has no batched entry point: cube by cube
-            ws1 = B.alloc_workspace(nx, ny, nz, 1)
-            for b, p in enumerate(plist):
-                B.idg_filter_pm(cur[b], n - done, p, out=cur[b], workspace=ws1)
-        else:
-            B.idg_filter_batched(cur, n - done, plist, out=cur, workspace=ws)
+        step = B.idg_filter_pm_batched if variant == "pm" else B.idg_filter_batched
+        step(cur, n - done, plist, out=cur, workspace=ws)
         done = n
         if n not in report:
             continue

@@ -63,3 +63,24 @@ def test_pm_config0_and_invariants(B, oracle):
     for p in ((3, 1, 0), (3, 2, 0), (3, 3, 0), (3, 4, 0), (5, 0, 0), (0, 0, 0)):
         plan(B, *p)
         assert torch.equal(B.idg_filter_pm(t, 7, B.Params()), ref), p
+
+
+def test_pm_batched(B, oracle):
+    """idg_filter_pm_batched: per-cube parameters and iteration counts (0 included), in place and not, under every plan;
+    each cube equals the single-cube call bit for bit and the oracle within the tolerance."""
+    rng = np.random.default_rng(77)
+    cubes = (rng.normal(0, 1, (5, 9, 20, 24)) + 6.0 * (rng.random((5, 9, 20, 24)) < 0.04)).astype(np.float32)
+    ns = [0, 1, 4, 7, 10]
+    ps = [B.Params(K=0.75 + 0.5 * b, tau=0.03, cx=4.0 + b % 3, cy=5.0, cz=6.0, rms=1.0) for b in range(5)]
+    t = torch.from_numpy(cubes).cuda()
+    for p in PLANS:
+        plan(B, *p)
+        out = B.idg_filter_pm_batched(t, ns, ps)
+        inpl = t.clone()
+        B.idg_filter_pm_batched(inpl, ns, ps, out=inpl)
+        for b in range(5):
+            assert torch.equal(out[b], B.idg_filter_pm(t[b], ns[b], ps[b])), (p, b)
+            assert torch.equal(out[b], inpl[b]), (p, b)
+            ref = oracle.pm_filter_oracle(cubes[b], ns[b], **ps[b].f32())
+            assert np.abs(out[b].cpu().numpy().astype(np.float64) - ref).max() <= TOL, (p, b)
+    plan(B, 0, 0, 0)
