@@ -148,28 +148,41 @@ class ClockSampler:
                 "sm_max_mhz": max(mx) if mx else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+class OracleBuffers:
+    """fp64 input, output and scratch of the oracle for `planes` planes of a cube, allocated and touched once, so that
+    a timed call measures the oracle's arithmetic and not the page faults of fresh multi-GB allocations."""
+
+    def __init__(self, cube: np.ndarray, planes: int):
+        self.a = np.ascontiguousarray(cube[:planes], dtype=np.float64)
+        self.out = np.zeros_like(self.a)
+        self.scratch = np.zeros_like(self.a)
+
+    def run(self, n_iter: int, prm: dict) -> float:
+        import oracle
+        t0 = time.perf_counter()
+        oracle.idg_filter_oracle_into(self.a, n_iter, self.out, self.scratch, **prm)
+        return time.perf_counter() - t0
+
+
 def oracle_rate(cube: np.ndarray, n_iter: int, target_s: float, prm: dict, threads=None):
-    """Time the oracle, as it stands, on a bounded sample: the first planes of the workload cube."""
+    """Time the oracle, as it stands, on a bounded sample: the first planes of the workload cube (buffers preallocated
+    and touched; the fp32 -> fp64 conversion of the input is outside the timed region)."""
     import oracle
     cores = oracle.set_threads(threads or os.cpu_count() or 1)
     nz, ny, nx = cube.shape
-    probe = cube[: min(nz, 4)]
-    t0 = time.perf_counter()
-    oracle.idg_filter_oracle(probe, 2, **prm)
-    rate = probe.size * 2 / max(time.perf_counter() - t0, 1e-6)          # voxel-iter/s, rough
+    probe = OracleBuffers(cube, min(nz, 8))
+    probe.run(2, prm)                                                      # threads and caches warm
+    rate = probe.a.size * 2 / max(probe.run(2, prm), 1e-6)                 # voxel-iter/s, rough
     planes = int(max(2, min(nz, target_s * rate / (ny * nx * n_iter))))
-    sample = cube[:planes]
-    t0 = time.perf_counter()
-    oracle.idg_filter_oracle(sample, n_iter, **prm)
-    dt = time.perf_counter() - t0
-    if dt < target_s / 3 and planes < nz:       # the 4-plane probe underestimates the rate: size the sample again
+    buf = OracleBuffers(cube, planes)
+    dt = buf.run(n_iter, prm)
+    if dt < target_s / 3 and planes < nz:       # the small probe underestimates the rate: size the sample again
         planes = int(min(nz, planes * target_s / max(dt, 1e-6)))
-        sample = cube[:planes]
-        t0 = time.perf_counter()
-        oracle.idg_filter_oracle(sample, n_iter, **prm)
-        dt = time.perf_counter() - t0
-    desc = f"first {planes} of {nz} planes ({nx}x{ny}x{planes} voxels), n={n_iter}, fp64, {dt:.1f} s"
-    return sample.size * n_iter / dt / 1e9, cores, desc, dt
+        buf = OracleBuffers(cube, planes)
+        dt = buf.run(n_iter, prm)
+    desc = (f"first {planes} of {nz} planes ({nx}x{ny}x{planes} voxels), n={n_iter}, fp64, {dt:.1f} s "
+            "(buffers preallocated; conversion to fp64 not timed)")
+    return buf.a.size * n_iter / dt / 1e9, cores, desc, dt
 
 
 def run_reference(args) -> None:
@@ -188,15 +201,14 @@ def run_reference(args) -> None:
     r, _, _, _ = oracle_rate(cube.data, n, 2.0, prm)
     budget = 150.0 / max(1, args.steps + args.warmup)
     planes = int(max(2, min(nz, budget * r * 1e9 / (ny * nx * n))))
-    sample = cube.data[:planes]
+    buf = OracleBuffers(cube.data, planes)
     for _ in range(args.warmup):
-        oracle.idg_filter_oracle(sample, n, **prm)
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        oracle.idg_filter_oracle(sample, n, **prm)
-    dt = (time.perf_counter() - t0) / args.steps
+        buf.run(n, prm)
+    dt = sum(buf.run(n, prm) for _ in range(args.steps)) / args.steps
+    sample = buf.a
     v = sample.size * n / dt / 1e9
-    desc = f"first {planes} of {nz} planes ({nx}x{ny}x{planes} voxels) per step, n={n}, fp64 oracle"
+    desc = (f"first {planes} of {nz} planes ({nx}x{ny}x{planes} voxels) per step, n={n}, fp64 oracle "
+            "(buffers preallocated; conversion to fp64 not timed)")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,

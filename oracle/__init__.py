@@ -101,6 +101,24 @@ def idg_filter_oracle(cube: np.ndarray, n_iter: int, K: float = 1.5, tau: float 
     return out
 
 
+def idg_filter_oracle_into(a64: np.ndarray, n_iter: int, out: np.ndarray, scratch: np.ndarray, K: float = 1.5,
+                           tau: float = 0.0325, cx: float = 5.0, cy: float = 5.0, cz: float = 5.0,
+                           rms: float = 1.0) -> np.ndarray:
+    """:func:`idg_filter_oracle` on caller-owned fp64 buffers (marshalling only, the same C routine): ``a64`` is the
+    input already in fp64, ``out`` receives I_n, ``scratch`` is the second Jacobi buffer; all C-contiguous, same
+    shape.  For timing the arithmetic without the conversion and the page faults of fresh multi-GB allocations."""
+    for b in (a64, out, scratch):
+        if b.dtype != np.float64 or not b.flags.c_contiguous or b.shape != a64.shape or b.ndim != 3:
+            raise ValueError("buffers must be C-contiguous float64 arrays of one 3-D shape")
+    nz, ny, nx = a64.shape
+    dp = ctypes.POINTER(ctypes.c_double)
+    rc = _load().idg_oracle_f64(a64.ctypes.data_as(dp), nx, ny, nz, int(n_iter), float(K), float(tau), float(cx),
+                                float(cy), float(cz), float(rms), out.ctypes.data_as(dp), scratch.ctypes.data_as(dp))
+    if rc != 0:
+        raise ValueError(f"idg_oracle_f64 rejected its arguments (rc={rc})")
+    return out
+
+
 def pm_filter_oracle(cube: np.ndarray, n_iter: int, K: float = 1.5, tau: float = 0.0325,
                      cx: float = 5.0, cy: float = 5.0, cz: float = 5.0, rms: float = 1.0) -> np.ndarray:
     """n_iter updates of the gradient-driven (Perona-Malik, Eq. 5) variant of Eq. 7 in fp64:

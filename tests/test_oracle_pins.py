@@ -213,3 +213,21 @@ def test_threads_do_not_change_results(oracle):
     oracle.set_threads(4)
     f4 = oracle.idg_filter_oracle(a, 6, **DEF)
     np.testing.assert_array_equal(f1, f4)
+
+
+def test_into_variant_is_the_same_routine(oracle):
+    """idg_filter_oracle_into (caller-owned fp64 buffers; bench.py times it) returns bit for bit what
+    idg_filter_oracle returns, leaves its input untouched, and rejects buffers of the wrong kind."""
+    rng = np.random.default_rng(12)
+    a = rng.normal(0, 2, (6, 7, 9)).astype(np.float32)
+    a64 = a.astype(np.float64)
+    keep = a64.copy()
+    out, scratch = np.empty_like(a64), np.empty_like(a64)
+    for n in (0, 1, 4, 7):
+        got = oracle.idg_filter_oracle_into(a64, n, out, scratch, K=1.5, tau=0.03, cx=5.0, cy=4.0, cz=6.0, rms=2.0)
+        assert got is out and np.array_equal(out, oracle.idg_filter_oracle(a, n, K=1.5, tau=0.03, cx=5.0, cy=4.0, cz=6.0, rms=2.0))
+        assert np.array_equal(a64, keep)
+    with pytest.raises(ValueError):
+        oracle.idg_filter_oracle_into(a64, 1, out.astype(np.float32), scratch)
+    with pytest.raises(ValueError):
+        oracle.idg_filter_oracle_into(a64, 1, out[:, :, :8], scratch)
